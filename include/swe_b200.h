@@ -1,0 +1,166 @@
+/* swe_b200.h -- C ABI of the B200-native shallow-water time-step library.
+ *
+ * What it computes: the explicit finite-volume time step of Delmas & Soulaimani,
+ * "Parallel high-order resolution of the Shallow-water equations on real large-scale meshes with
+ * complex bathymetries" (arxiv 2307.16758; citations below are PAPER.md:<line>), section 6.1-6.2,
+ * on an unstructured triangle mesh, in fp64, on ONE NVIDIA B200 (sm_100a):
+ *   eq. 1   state U=(h, hu, hv)
+ *   eq. 2   rotational invariance F.n = T^-1 G(T U)
+ *   eq. 3   finite-volume update over the three sides of a triangle
+ *   BCs     transmissive / imposed inflow Q / wall (Q=0)
+ *   eq. 5   CFL time step, d = radius of the inscribed circle
+ *   eq. 6-14  HLL / HLLC flux and wave-speed estimates
+ *   eq. 15-21 WAF flux, TVD weights, SUPERBEE A(r,c)
+ *   eq. 24-25 limiter semantics (beta=1 MINBEE) of the MUSCL slopes
+ *   hydrostatic reconstruction, bed-slope S_O and friction S_f sources (named at PAPER.md:281,
+ *   295, 422; formulas = DESIGN.md readings R12, R15); least-squares gradients and Heun RK2 for
+ *   MUSCL (BASELINE.json north_star); ghost layers, send list + contiguous receive range per
+ *   neighbour, send buffer refreshed on the GPU every step          PAPER.md:121-127, 141, 460.
+ *
+ * Conventions (every entry point):
+ *   - returns SWE_OK (0) or a negative SWE_ERR_* code; never throws across the ABI; the message of
+ *     the last failure on the calling thread is returned by swe_last_error();
+ *   - array arguments are caller-owned and only read (inputs) or written (outputs) during the
+ *     call; every array pointer may be a HOST pointer or a DEVICE pointer of the current CUDA
+ *     device (classified with cudaPointerGetAttributes), so a torch tensor's data_ptr() can be
+ *     passed straight through; outputs are caller-allocated with the stated length;
+ *   - the user's cell numbering (the order of `tri`) is preserved at the boundary: the internal
+ *     renumbering (space-filling curve) is invisible;
+ *   - all real data are IEEE double, all indices int32 (counts int64);
+ *   - there is no CPU fallback: without a CUDA device swe_mesh_create fails with SWE_ERR_CUDA.
+ */
+#ifndef SWE_B200_H
+#define SWE_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swe_ctx swe_ctx; /* opaque; owns every host and device allocation it makes */
+
+enum { SWE_OK = 0, SWE_ERR_ARG = -1, SWE_ERR_MESH = -2, SWE_ERR_CUDA = -3, SWE_ERR_STATE = -4,
+       SWE_ERR_NOMEM = -5 };
+/* scheme: first-order HLLC + Euler (eq. 6-14); MUSCL = least-squares gradients +
+ * cell limiter + HLLC + Heun RK2 (north_star); WAF + Euler (eq. 15-21). */
+enum { SWE_HLLC = 0, SWE_MUSCL = 1, SWE_WAF = 2 };
+/* boundary kinds (fixed level: PAPER.md:518, 548, reading R11) */
+enum { SWE_BC_WALL = 0, SWE_BC_INFLOW_Q = 1, SWE_BC_LEVEL = 2, SWE_BC_TRANSMISSIVE = 3 };
+enum { SWE_RENUM_NONE = 0, SWE_RENUM_HILBERT = 1 };
+
+/* Build the mesh (host: topology + geometry of SURVEY.md Appendix A.1, renumbering; then upload).
+ *   nv, x, y, zb : vertices, coordinates [m] and bed elevation [m] per vertex
+ *   nt, tri      : 3*nt vertex ids, any winding (re-oriented counter-clockwise internally)
+ *   nb, bedge, btag : nb tagged boundary edges as 2*nb vertex ids + nb tag ids (>=0); boundary edges
+ *                  not listed are walls.  Pointers may be NULL when nb == 0.
+ *   renumber     : SWE_RENUM_*
+ *   cuda_stream  : cudaStream_t the context will launch on (NULL = the legacy default stream)
+ * Errors: SWE_ERR_ARG (NULL / negative sizes), SWE_ERR_MESH (vertex id out of range, zero-area
+ * triangle, edge shared by more than two triangles, tagged edge that is not a boundary edge),
+ * SWE_ERR_CUDA (no device / allocation or copy failure).  Initial state: h = hu = hv = 0, t = 0.
+ * Defaults: g = 9.81, h_dry = 1e-6, h_thin = 1e-3, beta = 1, Manning n = 0, every tag = wall. */
+int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y, const double* zb,
+                    int64_t nt, const int32_t* tri, int64_t nb, const int32_t* bedge,
+                    const int32_t* btag, int renumber, void* cuda_stream);
+int swe_mesh_destroy(swe_ctx* ctx);
+/* any output pointer may be NULL.  min_inradius: eq. 5's d. */
+int swe_mesh_info(const swe_ctx* ctx, int64_t* ncell, int64_t* nedge, int64_t* nbedge,
+                  double* min_inradius);
+/* g [m/s2]; h_dry: wet threshold (wet <=> h > h_dry); h_thin: WAF falls back to HLLC within one
+ * cell of depth <= h_thin (reading R14); beta: limiter parameter, kappa = beta/2 (1 = minmod /
+ * MINBEE eq. 24, 2 = Barth-Jespersen, <= 0 = unlimited). */
+int swe_set_params(swe_ctx* ctx, double g, double h_dry, double h_thin, double beta);
+/* Manning n per cell, length nt, user order; NULL = 0 everywhere (no friction). */
+int swe_set_manning(swe_ctx* ctx, const double* n_cell);
+/* kind of the boundary edges carrying `tag` and its value: discharge Q [m3/s, into the domain,
+ * spread uniformly over the tag's total width] for SWE_BC_INFLOW_Q, free-surface level [m] for
+ * SWE_BC_LEVEL; ignored otherwise. */
+int swe_set_bc(swe_ctx* ctx, int tag, int kind, double value);
+/* state, nt values each, user order.  SWE_ERR_STATE if any h is NaN or negative.  Resets t to 0
+ * only if reset_time != 0 in swe_set_time; swe_set_state itself leaves t unchanged. */
+int swe_set_state(swe_ctx* ctx, const double* h, const double* hu, const double* hv);
+int swe_get_state(const swe_ctx* ctx, double* h, double* hu, double* hv);
+int swe_set_time(swe_ctx* ctx, double t);
+/* Advance nsteps time steps: per step dt = cfl * min_i R_i/lambda_i (eq. 5) by a device
+ * min-reduction, then the scheme's stage(s).  Asynchronous on the context's stream (dt never
+ * visits the host) unless t_out or last_dt_out is non-NULL (host pointers), in which case the
+ * call synchronises the stream and returns the simulated time and the last dt.  With zones built
+ * (swe_zones_create) the step runs zone-wise with pack/unpack of the ghost cells every stage.
+ * Errors: SWE_ERR_ARG (nsteps < 0, cfl <= 0, unknown scheme), SWE_ERR_STATE (zones built with too
+ * few ghost layers for the scheme: WAF needs 2), SWE_ERR_CUDA. */
+int swe_step(swe_ctx* ctx, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out);
+
+/* Zone decomposition resident on this GPU.
+ *   nzones : number of zones; zone_of_cell (nt, user order, values in [0,nzones)) or NULL =
+ *            recursive coordinate bisection (nzones must then be a power of two)
+ *   nlayers: ghost layers per zone, 1..3 (edge adjacency)
+ * Each zone gets its own copy of its owned + ghost cells; per (zone, source zone) one send list
+ * (indices into the source zone) and one contiguous receive range.  nzones == 0 removes zones. */
+int swe_zones_create(swe_ctx* ctx, int nzones, int nlayers, const int32_t* zone_of_cell);
+/* pack: send buffer[k] = U[send_idx[k]] for every link whose SOURCE is `zone` (-1 = all zones);
+ * unpack: copy the buffers into the contiguous ghost ranges of `zone` (-1 = all). */
+int swe_pack_ghosts(swe_ctx* ctx, int zone);
+int swe_unpack_ghosts(swe_ctx* ctx, int zone);
+int swe_zone_stats(const swe_ctx* ctx, int64_t* send_cells_total, int64_t* bytes_per_exchange,
+                   int64_t* ghost_cells_total);
+/* description of one zone for tests and for a multi-GPU driver: counts, then the arrays.
+ * cells: user ids of owned cells then ghost blocks (nowned+nghost); layer: 0 owned, l = ghost
+ * layer; links (one per source zone, ascending): src zone, receive start, count; send list of a
+ * link = source-zone-local indices. */
+int swe_zone_describe(const swe_ctx* ctx, int zone, int64_t* nowned, int64_t* nghost, int64_t* nlinks);
+int swe_zone_cells(const swe_ctx* ctx, int zone, int32_t* cells, int32_t* layer);
+int swe_zone_links(const swe_ctx* ctx, int zone, int32_t* src, int32_t* start, int32_t* count);
+int swe_zone_sendlist(const swe_ctx* ctx, int zone, int link, int32_t* send_idx);
+
+/* ---- single passes of the hot path, exposed for parity tests and kernel timing -------------
+ * (SURVEY.md section 8(a) rows a2, a3-a7, a8, a9).  They act on the current state, un-zoned. */
+/* a9: dt = cfl * min over wet cells of R_i / (sqrt(g h) + |u|) (eq. 5); 0 if no wet cell. */
+int swe_compute_dt(swe_ctx* ctx, double cfl, double* dt_out /* host */);
+/* a2: limited least-squares gradients, out[8*nt], user order, per cell
+ * (eta_x, eta_y, h_x, h_y, u_x, u_y, v_x, v_y). */
+int swe_gradients(swe_ctx* ctx, double* out);
+/* a3-a7: fluxes of the current state with time step dt (dt only matters for WAF): per cell and
+ * local side k=0..2, sigma * Phi (3 components) as the cell sees it, out[9*nt], user order,
+ * out[9*i + 3*k + c]; local side k joins vertices k -> k+1 of the counter-clockwise triangle. */
+int swe_side_fluxes(swe_ctx* ctx, double dt, int scheme, double* out);
+/* a8 (+a2..a7): one Euler stage with a given dt from the current state, result to caller arrays
+ * (nt each, user order); the context's state is not changed. */
+int swe_euler_stage(swe_ctx* ctx, double dt, int scheme, double* h1, double* hu1, double* hv1);
+/* counters: steps taken, kernels launched by this context so far, bytes moved by pack+unpack. */
+int swe_get_stats(const swe_ctx* ctx, int64_t* steps, int64_t* kernel_launches, int64_t* halo_bytes);
+/* time the hot path with CUDA events on the context's stream: runs swe_step(nsteps,...) between
+ * two events and returns the elapsed milliseconds (synchronises). */
+int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_out);
+/* per-kernel timing: runs `reps` launches of one kernel of the hot path on the current state
+ * between two events; which: 0 dt_reduce, 1 grad_limit, 2 edge_flux(scheme), 3 cell_update (Euler
+ * stage), 4 cell_update (Heun combine), 5 pack, 6 unpack.  The state is left unchanged (updates
+ * write to the stage buffer). */
+int swe_kernel_timed(swe_ctx* ctx, int which, int scheme, int reps, float* ms_out);
+
+/* per-kernel timing inside swe_step: with profiling on, every kernel launch of swe_step is
+ * bracketed by two CUDA events on the context's stream; swe_get_profile synchronises and returns
+ * accumulated milliseconds and launch counts per kind (7 each):
+ * 0 dt_reduce, 1 grad_limit, 2 edge_flux, 3 cell_update, 4 pack, 5 unpack, 6 dt_finalize. */
+int swe_set_profile(swe_ctx* ctx, int on);
+int swe_get_profile(swe_ctx* ctx, double* ms, int64_t* count);
+
+const char* swe_last_error(void); /* thread-local, static storage */
+
+/* ---- host-only inspection of the set-up (no GPU needed; used by the CPU test-suite) ----------
+ * swe_host_mesh_build runs the same host set-up as swe_mesh_create (topology, geometry of
+ * SURVEY.md A.1, renumbering) and swe_host_zones_build the zone builder of A.12, without touching
+ * a device.  swe_host_get copies a named array out (see csrc/host_inspect.cpp for the names) and
+ * returns its element count (-1 capacity too small, -2 unknown name). */
+int swe_host_mesh_build(void** out, int64_t nv, const double* x, const double* y, const double* zb,
+                        int64_t nt, const int32_t* tri, int64_t nb, const int32_t* bedge,
+                        const int32_t* btag, int renumber);
+int swe_host_zones_build(void* handle, int nzones, int nlayers, const int32_t* zone_of_cell);
+void swe_host_mesh_free(void* handle);
+int64_t swe_host_get(void* handle, const char* name, void* out, int64_t capacity_bytes);
+const char* swe_host_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWE_B200_H */

@@ -1,0 +1,481 @@
+// host_mesh.cpp -- host set-up: mesh topology / geometry (following the
+// paper's "cell-to-cell adjacency from an edge map" PAPER.md:74), Hilbert renumbering for gather
+// locality (BASELINE.json north_star), zone decomposition with ghost layers and send / receive
+// lists (A.12).  Not on the timed path.
+#include "host_mesh.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+namespace swe {
+namespace {
+
+// Hilbert curve index of integer point (px,py) on an n x n lattice, n = 2^order.
+inline uint64_t hilbert_d(uint32_t order, uint32_t px, uint32_t py) {
+    const uint32_t n = 1u << order;
+    uint64_t d = 0;
+    for (uint32_t s = n >> 1; s > 0; s >>= 1) {
+        uint32_t rx = (px & s) ? 1u : 0u, ry = (py & s) ? 1u : 0u;
+        d += (uint64_t)s * (uint64_t)s * (uint64_t)((3u * rx) ^ ry);
+        if (ry == 0) {
+            if (rx == 1) { px = n - 1 - px; py = n - 1 - py; }
+            std::swap(px, py);
+        }
+    }
+    return d;
+}
+
+struct HalfEdge { int32_t hi; int32_t slot; };
+
+}  // namespace
+
+bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, const double* zb,
+                     int64_t nt, const int32_t* tri_in, int64_t nb, const int32_t* bedge,
+                     const int32_t* btag, int renumber, std::string& err) {
+    H = HostMesh();
+    H.nv = nv; H.nt = nt;
+    if (nt > (int64_t)700000000) { err = "too many cells for int32 side indices"; return false; }
+    std::vector<int32_t> tri(tri_in, tri_in + 3 * nt);
+    for (int64_t i = 0; i < 3 * nt; ++i)
+        if (tri[i] < 0 || tri[i] >= nv) { err = "triangle vertex id out of range"; return false; }
+
+    // ---- A.1.1 / A.1.3 : orientation, area, centroid, cell bed (user numbering) ----
+    std::vector<double> area(nt), ucx(nt), ucy(nt), uzc(nt);
+    for (int64_t i = 0; i < nt; ++i) {
+        int32_t* v = &tri[3 * i];
+        double x0 = x[v[0]], y0 = y[v[0]];
+        double a = 0.5 * ((x[v[1]] - x0) * (y[v[2]] - y0) - (x[v[2]] - x0) * (y[v[1]] - y0));
+        if (a < 0.0) {
+            std::swap(v[1], v[2]);
+            a = 0.5 * ((x[v[1]] - x0) * (y[v[2]] - y0) - (x[v[2]] - x0) * (y[v[1]] - y0));
+        }
+        if (!(a > 0.0)) { err = "degenerate (zero-area) triangle"; return false; }
+        area[i] = a;
+        ucx[i] = (x[v[0]] + x[v[1]] + x[v[2]]) / 3.0;
+        ucy[i] = (y[v[0]] + y[v[1]] + y[v[2]]) / 3.0;
+        uzc[i] = (zb[v[0]] + zb[v[1]] + zb[v[2]]) / 3.0;
+    }
+
+    // ---- A.1.2 : global edges = distinct vertex pairs.  Counting sort of the 3*nt cell sides by
+    // their lower vertex id, then pairing inside each bucket by the higher vertex id. ----
+    const int64_t ns = 3 * nt;
+    std::vector<int64_t> boff(nv + 1, 0);
+    auto side_lo_hi = [&](int64_t s, int32_t& lo, int32_t& hi) {
+        int64_t i = s / 3; int k = (int)(s % 3);
+        int32_t a = tri[3 * i + k], b = tri[3 * i + (k + 1) % 3];
+        lo = std::min(a, b); hi = std::max(a, b);
+    };
+    for (int64_t s = 0; s < ns; ++s) { int32_t lo, hi; side_lo_hi(s, lo, hi); boff[lo + 1]++; }
+    for (int64_t v = 0; v < nv; ++v) boff[v + 1] += boff[v];
+    std::vector<HalfEdge> he(ns);
+    {
+        std::vector<int64_t> fill(boff.begin(), boff.end() - 1);
+        for (int64_t s = 0; s < ns; ++s) {  // ascending slot => ascending user cell id per bucket
+            int32_t lo, hi; side_lo_hi(s, lo, hi);
+            if (lo == hi) { err = "triangle repeats a vertex"; return false; }
+            he[fill[lo]++] = HalfEdge{hi, (int32_t)s};
+        }
+    }
+    // user-level edges: slot of the L side (smaller user cell id, A.1.4) and of the R side (-1)
+    std::vector<int32_t> esL, esR;
+    esL.reserve(ns / 2 + nt / 8 + 16); esR.reserve(ns / 2 + nt / 8 + 16);
+    std::vector<int32_t> side_edge(ns, -1);
+    for (int64_t v = 0; v < nv; ++v) {
+        HalfEdge* b = he.data() + boff[v];
+        int64_t n = boff[v + 1] - boff[v];
+        std::sort(b, b + n, [](const HalfEdge& p, const HalfEdge& q) {
+            return p.hi != q.hi ? p.hi < q.hi : p.slot < q.slot; });
+        for (int64_t j = 0; j < n;) {
+            int64_t j2 = j + 1;
+            while (j2 < n && b[j2].hi == b[j].hi) ++j2;
+            if (j2 - j > 2) { err = "non-manifold edge (more than two triangles)"; return false; }
+            int32_t e = (int32_t)esL.size();
+            esL.push_back(b[j].slot);
+            esR.push_back(j2 - j == 2 ? b[j + 1].slot : -1);
+            side_edge[b[j].slot] = e;
+            if (j2 - j == 2) {
+                if (b[j].slot / 3 == b[j + 1].slot / 3) { err = "triangle uses an edge twice"; return false; }
+                side_edge[b[j + 1].slot] = e;
+            }
+            j = j2;
+        }
+    }
+    const int64_t ne = (int64_t)esL.size();
+
+    // ---- A.1.4 / A.1.6 : edge geometry from the end points a->b as traversed by the L-cell ----
+    std::vector<double> elen(ne), enx(ne), eny(ne), edx(ne), rlx(ne), rly(ne), rrx(ne), rry(ne);
+    std::vector<int32_t> utag(ne, -1);
+    int64_t nbe = 0;
+    for (int64_t e = 0; e < ne; ++e) {
+        int64_t L = esL[e] / 3; int kL = esL[e] % 3;
+        int32_t a = tri[3 * L + kL], b = tri[3 * L + (kL + 1) % 3];
+        double dx = x[b] - x[a], dy = y[b] - y[a];
+        double len = std::sqrt(dx * dx + dy * dy);
+        double n1 = dy / len, n2 = -dx / len;
+        double mx = 0.5 * (x[a] + x[b]), my = 0.5 * (y[a] + y[b]);
+        elen[e] = len; enx[e] = n1; eny[e] = n2;
+        rlx[e] = mx - ucx[L]; rly[e] = my - ucy[L];
+        if (esR[e] >= 0) {
+            int64_t R = esR[e] / 3;
+            rrx[e] = mx - ucx[R]; rry[e] = my - ucy[R];
+            edx[e] = (rlx[e] * n1 + rly[e] * n2) - (rrx[e] * n1 + rry[e] * n2);
+        } else {
+            rrx[e] = 0.0; rry[e] = 0.0;
+            edx[e] = 2.0 * (rlx[e] * n1 + rly[e] * n2);
+            ++nbe;
+        }
+    }
+    H.nbe = nbe;
+
+    // ---- boundary tags: look the pair up in its lower vertex's bucket ----
+    for (int64_t j = 0; j < nb; ++j) {
+        int32_t a = bedge[2 * j], b = bedge[2 * j + 1];
+        if (a < 0 || b < 0 || a >= nv || b >= nv) { err = "boundary edge vertex id out of range"; return false; }
+        if (btag[j] < 0) { err = "negative boundary tag"; return false; }
+        int32_t lo = std::min(a, b), hi = std::max(a, b);
+        int32_t e = -1;
+        for (int64_t q = boff[lo]; q < boff[lo + 1]; ++q)
+            if (he[q].hi == hi) { e = side_edge[he[q].slot]; break; }
+        if (e < 0 || esR[e] >= 0) { err = "tagged edge is not a boundary edge"; return false; }
+        utag[e] = btag[j];
+    }
+    he.clear(); he.shrink_to_fit();
+    boff.clear(); boff.shrink_to_fit();
+
+    // ---- renumbering: Hilbert curve through the centroids (ties by user id) ----
+    std::vector<int32_t> cell_user(nt);
+    std::iota(cell_user.begin(), cell_user.end(), 0);
+    if (renumber == 1 && nt > 1) {
+        double xmin = ucx[0], xmax = ucx[0], ymin = ucy[0], ymax = ucy[0];
+        for (int64_t i = 1; i < nt; ++i) {
+            xmin = std::min(xmin, ucx[i]); xmax = std::max(xmax, ucx[i]);
+            ymin = std::min(ymin, ucy[i]); ymax = std::max(ymax, ucy[i]);
+        }
+        const uint32_t order = 24;
+        double ext = std::max(xmax - xmin, ymax - ymin);
+        double sc = ext > 0.0 ? ((double)((1u << order) - 1)) / ext : 0.0;
+        std::vector<uint64_t> key(nt);
+        for (int64_t i = 0; i < nt; ++i) {
+            uint32_t px = (uint32_t)((ucx[i] - xmin) * sc), py = (uint32_t)((ucy[i] - ymin) * sc);
+            uint64_t d = hilbert_d(order, px, py);
+            key[i] = d;
+        }
+        std::sort(cell_user.begin(), cell_user.end(), [&](int32_t a, int32_t b) {
+            return key[a] != key[b] ? key[a] < key[b] : a < b; });
+    }
+    H.user_cell.resize(nt);
+    for (int64_t i = 0; i < nt; ++i) H.user_cell[cell_user[i]] = (int32_t)i;
+
+    // ---- edge order: interior edges by their lower device cell id, boundary edges last ----
+    std::vector<int32_t> eorder(ne);   // device edge id -> user-level edge id
+    {
+        std::vector<int64_t> cnt(nt + 1, 0);
+        std::vector<int32_t> kmin(ne), kmax(ne);
+        for (int64_t e = 0; e < ne; ++e) {
+            int32_t dl = H.user_cell[esL[e] / 3];
+            int32_t dr = esR[e] >= 0 ? H.user_cell[esR[e] / 3] : dl;
+            kmin[e] = std::min(dl, dr); kmax[e] = std::max(dl, dr);
+        }
+        // pass 1: interior
+        int64_t pos = 0;
+        for (int pass = 0; pass < 2; ++pass) {
+            std::fill(cnt.begin(), cnt.end(), 0);
+            for (int64_t e = 0; e < ne; ++e)
+                if ((esR[e] >= 0) == (pass == 0)) cnt[kmin[e] + 1]++;
+            for (int64_t i = 0; i < nt; ++i) cnt[i + 1] += cnt[i];
+            int64_t total = cnt[nt];
+            std::vector<int64_t> fill(cnt.begin(), cnt.end() - 1);
+            for (int64_t e = 0; e < ne; ++e)
+                if ((esR[e] >= 0) == (pass == 0)) eorder[pos + fill[kmin[e]]++] = (int32_t)e;
+            for (int64_t i = 0; i < nt; ++i) {   // at most 3 per bucket: order by the higher cell id
+                int32_t* b = eorder.data() + pos + cnt[i];
+                int64_t n = cnt[i + 1] - cnt[i];
+                std::sort(b, b + n, [&](int32_t p, int32_t q) {
+                    return kmax[p] != kmax[q] ? kmax[p] < kmax[q] : p < q; });
+            }
+            pos += total;
+        }
+    }
+    std::vector<int32_t> edev(ne);     // user-level edge id -> device edge id
+    for (int64_t e = 0; e < ne; ++e) edev[eorder[e]] = (int32_t)e;
+
+    // ---- fill the device-numbered arrays ----
+    MeshArrays& M = H.m;
+    M.nc = nt; M.ne = ne; M.ne_int = ne - nbe;
+    M.cell_user = cell_user;
+    M.c2c.assign(4 * nt, 0); M.c2e.assign(4 * nt, 0);
+    M.zc.resize(nt); M.area.resize(nt); M.rin.resize(nt);
+    for (int k = 0; k < 3; ++k) { M.w[k].resize(2 * nt); M.r[k].resize(2 * nt); }
+    M.elr.resize(2 * ne); M.en.resize(2 * ne); M.elen.resize(ne); M.edx.resize(ne);
+    M.erl.resize(2 * ne); M.err.resize(2 * ne);
+    M.btag.assign(nbe, -1);
+    H.cx.resize(nt); H.cy.resize(nt);
+    for (int64_t d = 0; d < ne; ++d) {
+        int32_t e = eorder[d];
+        M.elr[2 * d] = H.user_cell[esL[e] / 3];
+        M.elr[2 * d + 1] = esR[e] >= 0 ? H.user_cell[esR[e] / 3] : -1;
+        M.en[2 * d] = enx[e]; M.en[2 * d + 1] = eny[e];
+        M.elen[d] = elen[e]; M.edx[d] = edx[e];
+        M.erl[2 * d] = rlx[e]; M.erl[2 * d + 1] = rly[e];
+        M.err[2 * d] = rrx[e]; M.err[2 * d + 1] = rry[e];
+        if (d >= M.ne_int) M.btag[d - M.ne_int] = utag[e];
+    }
+    double min_rin = 1e300;
+    for (int64_t i = 0; i < nt; ++i) {
+        int64_t u = cell_user[i];
+        M.zc[i] = uzc[u]; M.area[i] = area[u];
+        H.cx[i] = ucx[u]; H.cy[i] = ucy[u];
+        double rx[3], ry[3], nox[3], noy[3], dxk[3], dyk[3], lk[3];
+        for (int k = 0; k < 3; ++k) {
+            int32_t e = side_edge[3 * u + k];
+            bool isL = (esL[e] == 3 * u + k);
+            lk[k] = elen[e];
+            if (isL) { rx[k] = rlx[e]; ry[k] = rly[e]; nox[k] = enx[e]; noy[k] = eny[e]; }
+            else { rx[k] = rrx[e]; ry[k] = rry[e]; nox[k] = -enx[e]; noy[k] = -eny[e]; }
+            int32_t other = isL ? esR[e] : esL[e];
+            int32_t d = edev[e];
+            M.c2e[4 * i + k] = isL ? d : ~d;
+            if (other >= 0) {
+                int64_t un = other / 3;
+                M.c2c[4 * i + k] = H.user_cell[un];
+                dxk[k] = ucx[un] - ucx[u];                    // A.1.7
+                dyk[k] = ucy[un] - ucy[u];
+            } else {
+                M.c2c[4 * i + k] = -1 - d;
+                double rn = rx[k] * nox[k] + ry[k] * noy[k];  // mirror point across the boundary edge
+                dxk[k] = 2.0 * rn * nox[k];
+                dyk[k] = 2.0 * rn * noy[k];
+            }
+            M.r[k][2 * i] = rx[k]; M.r[k][2 * i + 1] = ry[k];
+        }
+        M.rin[i] = 2.0 * area[u] / (lk[0] + lk[1] + lk[2]);   // A.1.5
+        min_rin = std::min(min_rin, M.rin[i]);
+        double a11 = 0.0, a12 = 0.0, a22 = 0.0;
+        for (int k = 0; k < 3; ++k) { a11 += dxk[k] * dxk[k]; a12 += dxk[k] * dyk[k]; a22 += dyk[k] * dyk[k]; }
+        double det = a11 * a22 - a12 * a12;
+        for (int k = 0; k < 3; ++k) {
+            M.w[k][2 * i] = (a22 * dxk[k] - a12 * dyk[k]) / det;
+            M.w[k][2 * i + 1] = (-a12 * dxk[k] + a11 * dyk[k]) / det;
+        }
+    }
+    H.min_rin = nt > 0 ? min_rin : 0.0;
+
+    // distinct tags and their widths (sum of edge lengths, reading R10)
+    for (int64_t b = 0; b < nbe; ++b) {
+        int32_t t = M.btag[b];
+        if (t < 0) continue;
+        size_t j = 0;
+        for (; j < H.tags.size(); ++j) if (H.tags[j] == t) break;
+        if (j == H.tags.size()) { H.tags.push_back(t); H.tag_width.push_back(0.0); }
+    }
+    // widths summed in USER-LEVEL edge order so they do not depend on the renumbering
+    for (int64_t e = 0; e < ne; ++e) {
+        if (esR[e] >= 0 || utag[e] < 0) continue;
+        for (size_t j = 0; j < H.tags.size(); ++j)
+            if (H.tags[j] == utag[e]) { H.tag_width[j] += elen[e]; break; }
+    }
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// zones (A.12)
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+void rcb_split(const HostMesh& H, std::vector<int32_t>& ids, int z0, int nz, std::vector<int32_t>& zone_of) {
+    if (nz == 1) { for (int32_t i : ids) zone_of[i] = z0; return; }
+    double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+    for (int32_t i : ids) {
+        xmin = std::min(xmin, H.cx[i]); xmax = std::max(xmax, H.cx[i]);
+        ymin = std::min(ymin, H.cy[i]); ymax = std::max(ymax, H.cy[i]);
+    }
+    const std::vector<double>& key = ((xmax - xmin) >= (ymax - ymin)) ? H.cx : H.cy;
+    const std::vector<int32_t>& uid = H.m.cell_user;
+    size_t nl = ids.size() / 2;
+    auto cmp = [&](int32_t a, int32_t b) { return key[a] != key[b] ? key[a] < key[b] : uid[a] < uid[b]; };
+    std::nth_element(ids.begin(), ids.begin() + nl, ids.end(), cmp);  // lower floor(n/2) go left
+    std::vector<int32_t> left(ids.begin(), ids.begin() + nl), right(ids.begin() + nl, ids.end());
+    ids.clear(); ids.shrink_to_fit();
+    rcb_split(H, left, z0, nz / 2, zone_of);
+    rcb_split(H, right, z0 + nz / 2, nz / 2, zone_of);
+}
+
+}  // namespace
+
+bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32_t* zone_of_cell_user,
+                 std::string& err) {
+    const MeshArrays& G = H.m;
+    const int64_t nc = G.nc;
+    Z = ZoneSet();
+    if (nz < 1) { err = "nzones must be >= 1"; return false; }
+    if (nlayers < 1 || nlayers > 3) { err = "nlayers must be 1, 2 or 3"; return false; }
+    Z.nz = nz; Z.nlayers = nlayers;
+    Z.zone_of.assign(nc, -1);
+    if (zone_of_cell_user) {
+        for (int64_t i = 0; i < nc; ++i) {
+            int32_t zc = zone_of_cell_user[G.cell_user[i]];
+            if (zc < 0 || zc >= nz) { err = "zone_of_cell value out of range"; return false; }
+            Z.zone_of[i] = zc;
+        }
+    } else {
+        if (nz & (nz - 1)) { err = "recursive coordinate bisection needs a power-of-two nzones"; return false; }
+        std::vector<int32_t> ids(nc);
+        std::iota(ids.begin(), ids.end(), 0);
+        rcb_split(H, ids, 0, nz, Z.zone_of);
+    }
+    Z.z.assign(nz, ZoneDesc());
+    std::vector<int32_t> owned_pos(nc);
+    for (int64_t i = 0; i < nc; ++i) {          // owned cells in ascending device id
+        ZoneDesc& zd = Z.z[Z.zone_of[i]];
+        owned_pos[i] = (int32_t)zd.cells.size();
+        zd.cells.push_back((int32_t)i);
+    }
+    // A.12.2 ghost layers by breadth-first search over edge adjacency; A.12.3 numbering
+    std::vector<int32_t> mark(nc, -1);
+    struct Gh { int32_t cell, layer, src; };
+    for (int zi = 0; zi < nz; ++zi) {
+        ZoneDesc& zd = Z.z[zi];
+        zd.nowned = (int64_t)zd.cells.size();
+        zd.layer.assign(zd.cells.size(), 0);
+        for (int32_t i : zd.cells) mark[i] = zi;
+        std::vector<int32_t> frontier = zd.cells, next;
+        std::vector<Gh> ghosts;
+        for (int l = 1; l <= nlayers; ++l) {
+            next.clear();
+            for (int32_t i : frontier)
+                for (int k = 0; k < 3; ++k) {
+                    int32_t nbq = G.c2c[4 * (int64_t)i + k];
+                    if (nbq >= 0 && mark[nbq] != zi) {
+                        mark[nbq] = zi; next.push_back(nbq);
+                        ghosts.push_back(Gh{nbq, l, Z.zone_of[nbq]});
+                    }
+                }
+            frontier.swap(next);
+        }
+        std::sort(ghosts.begin(), ghosts.end(), [](const Gh& a, const Gh& b) {
+            if (a.src != b.src) return a.src < b.src;
+            if (a.layer != b.layer) return a.layer < b.layer;
+            return a.cell < b.cell; });
+        for (const Gh& gq : ghosts) {
+            if (zd.links.empty() || zd.links.back().src != gq.src) {
+                ZoneLink lk; lk.src = gq.src; lk.start = (int32_t)zd.cells.size(); lk.count = 0;
+                zd.links.push_back(lk);
+            }
+            ZoneLink& lk = zd.links.back();
+            lk.count++;
+            lk.send.push_back(owned_pos[gq.cell]);
+            zd.cells.push_back(gq.cell);
+            zd.layer.push_back(gq.layer);
+        }
+    }
+    int64_t off = 0;
+    for (ZoneDesc& zd : Z.z) { zd.offset = off; off += (int64_t)zd.cells.size(); }
+    const int64_t ncz = off;
+    if (ncz > (int64_t)INT32_MAX / 4) { err = "zoned mesh too large"; return false; }
+
+    // ---- concatenated zoned mesh ----
+    const int gl = (nlayers >= 2) ? 1 : 0;   // gradients are needed on layers <= gl (A.12.5)
+    MeshArrays& M = Z.mesh;
+    M.nc = ncz;
+    M.cell_user.resize(ncz); M.c2c.assign(4 * ncz, 0); M.c2e.assign(4 * ncz, 0);
+    M.zc.resize(ncz); M.area.resize(ncz); M.rin.resize(ncz);
+    for (int k = 0; k < 3; ++k) { M.w[k].resize(2 * ncz); M.r[k].resize(2 * ncz); }
+    Z.src_of_cell.resize(ncz);
+    std::vector<int32_t> loc(nc, -1);
+    std::vector<int32_t> emark(G.ne, -1);
+    std::vector<std::vector<int32_t>> zint(nz), zbnd(nz);   // global edge ids per zone
+    for (int zi = 0; zi < nz; ++zi) {
+        ZoneDesc& zd = Z.z[zi];
+        for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = (int32_t)j;
+        // interior edges touching an owned cell, in the order the owned cells meet them
+        for (int64_t j = 0; j < zd.nowned; ++j) {
+            int32_t g = zd.cells[j];
+            for (int k = 0; k < 3; ++k) {
+                int32_t ce = G.c2e[4 * (int64_t)g + k];
+                int32_t e = ce >= 0 ? ce : ~ce;
+                if (e < G.ne_int && emark[e] != zi) { emark[e] = zi; zint[zi].push_back(e); }
+            }
+        }
+        // boundary edges of every cell whose gradient is evaluated
+        for (size_t j = 0; j < zd.cells.size(); ++j) {
+            if (zd.layer[j] > gl) continue;
+            int32_t g = zd.cells[j];
+            for (int k = 0; k < 3; ++k) {
+                int32_t nbq = G.c2c[4 * (int64_t)g + k];
+                if (nbq < 0) zbnd[zi].push_back(-1 - nbq);
+            }
+        }
+        for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = -1;
+    }
+    std::vector<int64_t> ioff(nz + 1, 0), boff(nz + 1, 0);
+    for (int zi = 0; zi < nz; ++zi) { ioff[zi + 1] = ioff[zi] + (int64_t)zint[zi].size(); boff[zi + 1] = boff[zi] + (int64_t)zbnd[zi].size(); }
+    M.ne_int = ioff[nz];
+    M.ne = M.ne_int + boff[nz];
+    if (M.ne > (int64_t)INT32_MAX / 2) { err = "zoned mesh too large"; return false; }
+    M.elr.resize(2 * M.ne); M.en.resize(2 * M.ne); M.elen.resize(M.ne); M.edx.resize(M.ne);
+    M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne);
+    M.btag.assign(M.ne - M.ne_int, -1);
+    std::vector<int32_t> eloc(G.ne, -1);
+    for (int zi = 0; zi < nz; ++zi) {
+        ZoneDesc& zd = Z.z[zi];
+        const int64_t o = zd.offset;
+        for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = (int32_t)j;
+        auto put_edge = [&](int64_t d, int32_t e) {
+            int32_t L = G.elr[2 * (int64_t)e], R = G.elr[2 * (int64_t)e + 1];
+            M.elr[2 * d] = (int32_t)(o + loc[L]);
+            M.elr[2 * d + 1] = R >= 0 ? (int32_t)(o + loc[R]) : -1;
+            M.en[2 * d] = G.en[2 * (int64_t)e]; M.en[2 * d + 1] = G.en[2 * (int64_t)e + 1];
+            M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e];
+            M.erl[2 * d] = G.erl[2 * (int64_t)e]; M.erl[2 * d + 1] = G.erl[2 * (int64_t)e + 1];
+            M.err[2 * d] = G.err[2 * (int64_t)e]; M.err[2 * d + 1] = G.err[2 * (int64_t)e + 1];
+            eloc[e] = (int32_t)d;
+        };
+        for (size_t q = 0; q < zint[zi].size(); ++q) put_edge(ioff[zi] + (int64_t)q, zint[zi][q]);
+        for (size_t q = 0; q < zbnd[zi].size(); ++q) {
+            int64_t d = M.ne_int + boff[zi] + (int64_t)q;
+            put_edge(d, zbnd[zi][q]);
+            M.btag[d - M.ne_int] = G.btag[zbnd[zi][q] - G.ne_int];
+        }
+        for (size_t j = 0; j < zd.cells.size(); ++j) {
+            const int64_t g = zd.cells[j], c = o + (int64_t)j;
+            const int lay = zd.layer[j];
+            M.cell_user[c] = G.cell_user[g];
+            Z.src_of_cell[c] = (int32_t)g;
+            M.zc[c] = G.zc[g]; M.area[c] = G.area[g]; M.rin[c] = G.rin[g];
+            for (int k = 0; k < 3; ++k) {
+                M.w[k][2 * c] = G.w[k][2 * g]; M.w[k][2 * c + 1] = G.w[k][2 * g + 1];
+                M.r[k][2 * c] = G.r[k][2 * g]; M.r[k][2 * c + 1] = G.r[k][2 * g + 1];
+                int32_t nbq = G.c2c[4 * g + k];
+                int32_t v;
+                if (nbq >= 0) v = loc[nbq] >= 0 ? (int32_t)(o + loc[nbq]) : NB_OUTSIDE;
+                else v = (lay <= gl) ? (-1 - eloc[-1 - nbq]) : NB_OUTSIDE;
+                M.c2c[4 * c + k] = v;
+                if (lay == 0) {
+                    int32_t ce = G.c2e[4 * g + k];
+                    int32_t e = ce >= 0 ? ce : ~ce;
+                    M.c2e[4 * c + k] = ce >= 0 ? eloc[e] : ~eloc[e];
+                }
+            }
+            M.c2c[4 * c + 3] = lay;
+            M.c2e[4 * c + 3] = lay;
+        }
+        for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = -1;
+    }
+    // ---- flattened exchange lists ----
+    Z.link_off.push_back(0);
+    for (int zi = 0; zi < nz; ++zi)
+        for (const ZoneLink& lk : Z.z[zi].links) {
+            for (int32_t j = 0; j < lk.count; ++j) {
+                Z.send_idx.push_back((int32_t)(Z.z[lk.src].offset + lk.send[j]));
+                Z.recv_idx.push_back((int32_t)(Z.z[zi].offset + lk.start + j));
+            }
+            Z.link_off.push_back((int64_t)Z.send_idx.size());
+            Z.link_src.push_back(lk.src);
+            Z.link_dst.push_back(zi);
+        }
+    return true;
+}
+
+}  // namespace swe

@@ -1,0 +1,840 @@
+// swe_api.cu -- C ABI of include/swe_b200.h: context, device memory, step scheduling.
+// Every step of the hot path runs in the kernels of swe_kernels.cuh; there is no CPU fallback.
+#include "../../include/swe_b200.h"
+#include "host_mesh.hpp"
+#include "swe_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace swe;
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+
+#define CU(call)                                                                        \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess)                                                          \
+            return fail(SWE_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+enum { KIND_DT = 0, KIND_GRAD = 1, KIND_FLUX = 2, KIND_UPDATE = 3, KIND_PACK = 4, KIND_UNPACK = 5,
+       KIND_MISC = 6, NKIND = 7 };
+
+// device copy of one MeshArrays + the state / gradient / flux buffers that live on it
+struct Store {
+    DevMesh dm{};
+    std::vector<void*> owned;          // every cudaMalloc of this store
+    int* d_cell_user = nullptr;
+    int* d_bkind = nullptr;
+    double* d_bval = nullptr;
+    double* d_nman = nullptr;
+    std::vector<int32_t> h_btag;
+    double4 *A = nullptr, *B = nullptr, *grad = nullptr;
+    FluxBuf F{};
+    int64_t nc = 0, ne = 0, nbe = 0;
+
+    template <class T> cudaError_t alloc(T** p, size_t n) {
+        void* q = nullptr;
+        cudaError_t e = cudaMalloc(&q, (n ? n : 1) * sizeof(T));
+        if (e == cudaSuccess) { owned.push_back(q); *p = (T*)q; }
+        return e;
+    }
+    template <class T> cudaError_t upload(T** p, const void* src, size_t n, cudaStream_t s) {
+        cudaError_t e = alloc(p, n);
+        if (e != cudaSuccess) return e;
+        if (n) e = cudaMemcpyAsync(*p, src, n * sizeof(T), cudaMemcpyHostToDevice, s);
+        return e;
+    }
+    void release() {
+        for (void* p : owned) cudaFree(p);
+        owned.clear();
+    }
+};
+
+}  // namespace
+
+struct swe_ctx {
+    cudaStream_t stream = nullptr;
+    int num_sm = 148;
+    HostMesh H;
+    ZoneSet Z;
+    bool has_zones = false;
+    Store g, z;
+    Par P{9.81, 1e-6, 1e-3, 0.5, 1};
+    double beta = 1.0;
+    std::map<int, std::pair<int, double>> bc;
+    StepScalars* d_S = nullptr;
+    bool min_valid = false;
+    int64_t launches = 0, halo_bytes = 0, steps = 0;
+    // zone exchange
+    int* d_send_idx = nullptr;
+    int* d_recv_idx = nullptr;
+    int* d_src_of_cell = nullptr;
+    double* d_sendbuf = nullptr;
+    int64_t nsend = 0;
+    // staging for host pointers
+    double* d_stage = nullptr;
+    size_t stage_elems = 0;
+    // profile
+    bool profile = false;
+    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> prof_events;
+    double prof_ms[NKIND] = {0};
+    int64_t prof_n[NKIND] = {0};
+    // grid sizes (persistent grid-stride kernels: a multiple of the SM count)
+    int grid_light = 148 * 8;
+    int grid_grad = 148 * 4, grid_flux[3] = {148 * 4, 148 * 2, 148 * 2}, grid_upd = 148 * 8;
+
+    Store& active() { return has_zones ? z : g; }
+};
+
+namespace {
+
+int grid_for(int64_t n, int cap) {
+    int64_t b = (n + 255) / 256;
+    if (b < 1) b = 1;
+    return (int)(b < cap ? b : cap);
+}
+
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <class F> void launch(swe_ctx* c, int kind, F&& f) {
+    if (c->profile) {
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        cudaEventRecord(a, c->stream);
+        f();
+        cudaEventRecord(b, c->stream);
+        c->prof_events.push_back({kind, {a, b}});
+    } else {
+        f();
+    }
+    c->launches++;
+}
+
+void profile_collect(swe_ctx* c) {
+    if (c->prof_events.empty()) return;
+    cudaStreamSynchronize(c->stream);
+    for (auto& pe : c->prof_events) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, pe.second.first, pe.second.second);
+        c->prof_ms[pe.first] += ms; c->prof_n[pe.first]++;
+        cudaEventDestroy(pe.second.first); cudaEventDestroy(pe.second.second);
+    }
+    c->prof_events.clear();
+}
+
+int ensure_stage(swe_ctx* c, size_t elems) {
+    if (c->stage_elems >= elems) return SWE_OK;
+    if (c->d_stage) cudaFree(c->d_stage);
+    c->d_stage = nullptr; c->stage_elems = 0;
+    CU(cudaMalloc((void**)&c->d_stage, elems * sizeof(double)));
+    c->stage_elems = elems;
+    return SWE_OK;
+}
+
+int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
+    cudaStream_t s = c->stream;
+    st.nc = M.nc; st.ne = M.ne; st.nbe = M.ne - M.ne_int;
+    st.h_btag = M.btag;
+    DevMesh& d = st.dm;
+    d.nc = (int)M.nc; d.ne = (int)M.ne; d.ne_int = (int)M.ne_int; d.glayer = 0;
+    int4* c2c; int4* c2e; double *zc, *area, *rin;
+    CU(st.upload(&c2c, M.c2c.data(), (size_t)M.nc, s));
+    CU(st.upload(&c2e, M.c2e.data(), (size_t)M.nc, s));
+    CU(st.upload(&zc, M.zc.data(), (size_t)M.nc, s));
+    CU(st.upload(&area, M.area.data(), (size_t)M.nc, s));
+    CU(st.upload(&rin, M.rin.data(), (size_t)M.nc, s));
+    d.c2c = c2c; d.c2e = c2e; d.zc = zc; d.area = area; d.rin = rin;
+    for (int k = 0; k < 3; ++k) {
+        double2 *w, *r;
+        CU(st.upload(&w, M.w[k].data(), (size_t)M.nc, s));
+        CU(st.upload(&r, M.r[k].data(), (size_t)M.nc, s));
+        d.w[k] = w; d.r[k] = r;
+    }
+    int2* elr; double2 *en, *erl, *err; double *elen, *edx;
+    CU(st.upload(&elr, M.elr.data(), (size_t)M.ne, s));
+    CU(st.upload(&en, M.en.data(), (size_t)M.ne, s));
+    CU(st.upload(&elen, M.elen.data(), (size_t)M.ne, s));
+    CU(st.upload(&edx, M.edx.data(), (size_t)M.ne, s));
+    CU(st.upload(&erl, M.erl.data(), (size_t)M.ne, s));
+    CU(st.upload(&err, M.err.data(), (size_t)M.ne, s));
+    d.elr = elr; d.en = en; d.elen = elen; d.edx = edx; d.erl = erl; d.err = err;
+    CU(st.upload(&st.d_cell_user, M.cell_user.data(), (size_t)M.nc, s));
+    CU(st.alloc(&st.d_bkind, (size_t)st.nbe));
+    CU(st.alloc(&st.d_bval, (size_t)st.nbe));
+    CU(st.alloc(&st.d_nman, (size_t)M.nc));
+    d.bkind = st.d_bkind; d.bval = st.d_bval; d.nman = st.d_nman;
+    d.layer = nullptr;
+    CU(st.alloc(&st.A, (size_t)M.nc));
+    CU(st.alloc(&st.B, (size_t)M.nc));
+    CU(st.alloc(&st.grad, 2 * (size_t)M.nc));
+    CU(st.alloc(&st.F.f1, (size_t)M.ne));
+    CU(st.alloc(&st.F.fxl, (size_t)M.ne));
+    CU(st.alloc(&st.F.fyl, (size_t)M.ne));
+    CU(st.alloc(&st.F.fxr, (size_t)M.ne));
+    CU(st.alloc(&st.F.fyr, (size_t)M.ne));
+    CU(cudaMemsetAsync(st.grad, 0, 2 * (size_t)M.nc * sizeof(double4), s));
+    CU(cudaMemsetAsync(st.B, 0, (size_t)M.nc * sizeof(double4), s));
+    CU(cudaMemsetAsync(st.d_nman, 0, (size_t)(M.nc ? M.nc : 1) * sizeof(double), s));
+    return SWE_OK;
+}
+
+// boundary kind / value per boundary edge from the tag table (A.8; inflow: q_n = -Q / W, R10)
+int refresh_bc(swe_ctx* c, Store& st) {
+    std::vector<int> kind(st.nbe, KB_WALL);
+    std::vector<double> val(st.nbe, 0.0);
+    for (int64_t b = 0; b < st.nbe; ++b) {
+        int t = st.h_btag[b];
+        if (t < 0) continue;
+        auto it = c->bc.find(t);
+        if (it == c->bc.end()) continue;
+        kind[b] = it->second.first;
+        if (kind[b] == KB_INFLOW) {
+            double w = 1.0;
+            for (size_t j = 0; j < c->H.tags.size(); ++j) if (c->H.tags[j] == t) w = c->H.tag_width[j];
+            val[b] = -it->second.second / w;
+        } else {
+            val[b] = it->second.second;
+        }
+    }
+    if (st.nbe) {
+        CU(cudaMemcpyAsync(st.d_bkind, kind.data(), st.nbe * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(st.d_bval, val.data(), st.nbe * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return SWE_OK;
+}
+
+__global__ void k_gather_cells(double4* __restrict__ dst, const double4* __restrict__ src,
+                               const int* __restrict__ idx, int n) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) dst[i] = src[idx[i]];
+}
+__global__ void k_gather_scalar(double* __restrict__ dst, const double* __restrict__ src,
+                                const int* __restrict__ idx, int n) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) dst[i] = src[idx[i]];
+}
+__global__ void k_scatter_owned(double4* __restrict__ dst, const double4* __restrict__ src,
+                                const int* __restrict__ idx, const uint8_t* __restrict__ layer, int n) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+        if (layer[i] == 0) dst[idx[i]] = src[i];
+}
+__global__ void k_reset_min(StepScalars* S) { S->min_bits = 0x7ff0000000000000ULL; }
+
+void free_zones(swe_ctx* c) {
+    c->z.release();
+    c->z = Store();
+    if (c->d_send_idx) cudaFree(c->d_send_idx);
+    if (c->d_recv_idx) cudaFree(c->d_recv_idx);
+    if (c->d_src_of_cell) cudaFree(c->d_src_of_cell);
+    if (c->d_sendbuf) cudaFree(c->d_sendbuf);
+    c->d_send_idx = c->d_recv_idx = c->d_src_of_cell = nullptr;
+    c->d_sendbuf = nullptr;
+    c->nsend = 0;
+    c->has_zones = false;
+    c->Z = ZoneSet();
+}
+
+// ---- kernel launch helpers (all on c->stream) ----
+void run_dt_reduce(swe_ctx* c, Store& st, const double4* U) {
+    launch(c, KIND_DT, [&] {
+        k_dt_reduce<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.dm, U, c->P, c->d_S);
+    });
+}
+void run_grad(swe_ctx* c, Store& st, const double4* U) {
+    launch(c, KIND_GRAD, [&] {
+        k_grad_limit<<<grid_for(st.nc, c->grid_grad), 256, 0, c->stream>>>(st.dm, U, st.grad, c->P);
+    });
+}
+void run_flux(swe_ctx* c, Store& st, const double4* U, int scheme) {
+    launch(c, KIND_FLUX, [&] {
+        const int gr = grid_for(st.ne, c->grid_flux[scheme]);
+        if (scheme == K_HLLC) k_edge_flux<K_HLLC><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else if (scheme == K_MUSCL) k_edge_flux<K_MUSCL><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else k_edge_flux<K_WAF><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+    });
+}
+// mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in
+void run_update(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout, int mode, bool fuse) {
+    launch(c, KIND_UPDATE, [&] {
+        const int gr = grid_for(st.nc, c->grid_upd);
+        if (mode == 0 && !fuse) k_cell_update<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
+        else if (mode == 0) k_cell_update<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
+        else if (!fuse) k_cell_update<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
+        else k_cell_update<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
+    });
+}
+void run_exchange_state(swe_ctx* c, double4* U, int64_t first, int64_t count, bool do_pack, bool do_unpack) {
+    if (count <= 0) return;
+    if (do_pack) {
+        launch(c, KIND_PACK, [&] {
+            k_pack_state<<<grid_for(count, c->grid_light), 256, 0, c->stream>>>(U, c->d_send_idx, c->d_sendbuf, first, count);
+        });
+        c->halo_bytes += count * (4 + 32 + 24);
+    }
+    if (do_unpack) {
+        launch(c, KIND_UNPACK, [&] {
+            k_unpack_state<<<grid_for(count, c->grid_light), 256, 0, c->stream>>>(U, c->d_recv_idx, c->d_sendbuf, c->z.dm.zc, first, count);
+        });
+        c->halo_bytes += count * (4 + 24 + 8 + 32);
+    }
+}
+void run_exchange_grad(swe_ctx* c) {
+    const int64_t count = c->nsend;
+    if (count <= 0) return;
+    launch(c, KIND_PACK, [&] {
+        k_pack_grad<<<grid_for(count, c->grid_light), 256, 0, c->stream>>>(c->z.grad, c->d_send_idx, (double4*)c->d_sendbuf, 0, count);
+    });
+    launch(c, KIND_UNPACK, [&] {
+        k_unpack_grad<<<grid_for(count, c->grid_light), 256, 0, c->stream>>>(c->z.grad, c->d_recv_idx, (const double4*)c->d_sendbuf, 0, count);
+    });
+    c->halo_bytes += count * (4 + 64 + 64 + 4 + 64 + 64);
+}
+
+// one Euler stage on the active store: [exchange] -> [grad (-> exchange grad)] -> flux -> update
+void run_stage(swe_ctx* c, Store& st, double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
+    if (c->has_zones) run_exchange_state(c, Uin, 0, c->nsend, true, true);
+    if (scheme == K_MUSCL) {
+        run_grad(c, st, Uin);
+        if (c->has_zones && c->Z.nlayers == 1) run_exchange_grad(c);
+    }
+    run_flux(c, st, Uin, scheme);
+    run_update(c, st, Uin, U0, Uout, mode, fuse);
+}
+
+int sync_global_from_zoned(swe_ctx* c) {
+    if (!c->has_zones) return SWE_OK;
+    k_scatter_owned<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->g.A, c->z.A, c->d_src_of_cell, c->z.dm.layer, (int)c->z.nc);
+    c->launches++;
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int check_ctx(const swe_ctx* c) { return c ? SWE_OK : fail(SWE_ERR_ARG, "null context"); }
+
+}  // namespace
+
+extern "C" {
+
+const char* swe_last_error(void) { return g_err.c_str(); }
+
+int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y, const double* zb,
+                    int64_t nt, const int32_t* tri, int64_t nb, const int32_t* bedge,
+                    const int32_t* btag, int renumber, void* cuda_stream) {
+    if (!out) return fail(SWE_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (nv <= 0 || nt <= 0 || !x || !y || !zb || !tri) return fail(SWE_ERR_ARG, "empty or NULL mesh arrays");
+    if (nb < 0 || (nb > 0 && (!bedge || !btag))) return fail(SWE_ERR_ARG, "bad boundary-edge arguments");
+    if (renumber != SWE_RENUM_NONE && renumber != SWE_RENUM_HILBERT) return fail(SWE_ERR_ARG, "unknown renumbering");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(SWE_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    // mesh arrays may be host or device pointers: bring device ones to the host for the set-up
+    std::vector<double> hx, hy, hz; std::vector<int32_t> ht, hb, hbt;
+    auto to_host_d = [&](const double* p, int64_t n, std::vector<double>& v) -> const double* {
+        if (!is_device_ptr(p)) return p;
+        v.resize(n); cudaMemcpy(v.data(), p, n * sizeof(double), cudaMemcpyDeviceToHost); return v.data(); };
+    auto to_host_i = [&](const int32_t* p, int64_t n, std::vector<int32_t>& v) -> const int32_t* {
+        if (!p || !is_device_ptr(p)) return p;
+        v.resize(n); cudaMemcpy(v.data(), p, n * sizeof(int32_t), cudaMemcpyDeviceToHost); return v.data(); };
+    x = to_host_d(x, nv, hx); y = to_host_d(y, nv, hy); zb = to_host_d(zb, nv, hz);
+    tri = to_host_i(tri, 3 * nt, ht); bedge = to_host_i(bedge, 2 * nb, hb); btag = to_host_i(btag, nb, hbt);
+
+    swe_ctx* c = new (std::nothrow) swe_ctx();
+    if (!c) return fail(SWE_ERR_NOMEM, "out of host memory");
+    c->stream = (cudaStream_t)cuda_stream;
+    std::string err;
+    bool ok = false;
+    try { ok = build_host_mesh(c->H, nv, x, y, zb, nt, tri, nb, bedge, btag, renumber, err); }
+    catch (const std::bad_alloc&) { delete c; return fail(SWE_ERR_NOMEM, "out of host memory in mesh set-up"); }
+    if (!ok) { delete c; return fail(SWE_ERR_MESH, err); }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) c->num_sm = prop.multiProcessorCount;
+    // persistent grids: (resident blocks per SM) x (SM count), from the occupancy calculator
+    auto occ = [&](const void* k, int fallback) {
+        int nbk = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k, 256, 0) != cudaSuccess || nbk < 1) { cudaGetLastError(); nbk = fallback; }
+        return nbk * c->num_sm;
+    };
+    c->grid_light = 8 * c->num_sm;
+    c->grid_grad = occ((const void*)k_grad_limit, 4);
+    c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC>, 4);
+    c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2);
+    c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2);
+    c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
+    int rc = upload_store(c, c->g, c->H.m);
+    if (rc == SWE_OK) {
+        cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
+        if (e != cudaSuccess) rc = fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    }
+    if (rc == SWE_OK) {
+        StepScalars s0; s0.min_bits = 0x7ff0000000000000ULL; s0.dt = 0.0; s0.t = 0.0; s0.last_dt = 0.0; s0.steps = 0;
+        cudaMemcpyAsync(c->d_S, &s0, sizeof(s0), cudaMemcpyHostToDevice, c->stream);
+        // initial state: h = hu = hv = 0, z = cell bed
+        k_fill<<<grid_for(4 * c->g.nc, c->grid_light), 256, 0, c->stream>>>((double*)c->g.A, 0.0, 4 * c->g.nc);
+        rc = refresh_bc(c, c->g);
+    }
+    if (rc == SWE_OK) {
+        // z component of the state records
+        cudaError_t e = cudaMemcpy2DAsync((char*)c->g.A + 3 * sizeof(double), sizeof(double4), c->g.dm.zc, sizeof(double),
+                                          sizeof(double), (size_t)c->g.nc, cudaMemcpyDeviceToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync((char*)c->g.B + 3 * sizeof(double), sizeof(double4), c->g.dm.zc, sizeof(double),
+                                                    sizeof(double), (size_t)c->g.nc, cudaMemcpyDeviceToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    }
+    if (rc != SWE_OK) { std::string keep = g_err; swe_mesh_destroy(c); g_err = keep; return rc; }
+    *out = c;
+    return SWE_OK;
+}
+
+int swe_mesh_destroy(swe_ctx* c) {
+    if (!c) return SWE_OK;
+    cudaStreamSynchronize(c->stream);
+    for (auto& pe : c->prof_events) { cudaEventDestroy(pe.second.first); cudaEventDestroy(pe.second.second); }
+    free_zones(c);
+    c->g.release();
+    if (c->d_S) cudaFree(c->d_S);
+    if (c->d_stage) cudaFree(c->d_stage);
+    delete c;
+    return SWE_OK;
+}
+
+int swe_mesh_info(const swe_ctx* c, int64_t* ncell, int64_t* nedge, int64_t* nbedge, double* min_inradius) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (ncell) *ncell = c->H.nt;
+    if (nedge) *nedge = c->H.m.ne;
+    if (nbedge) *nbedge = c->H.nbe;
+    if (min_inradius) *min_inradius = c->H.min_rin;
+    return SWE_OK;
+}
+
+int swe_set_params(swe_ctx* c, double g, double h_dry, double h_thin, double beta) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!(g > 0.0) || !(h_dry >= 0.0) || !(h_thin >= 0.0) || beta != beta) return fail(SWE_ERR_ARG, "bad parameter value");
+    c->P.g = g; c->P.h_dry = h_dry; c->P.h_thin = h_thin; c->beta = beta;
+    c->P.kappa = beta / 2.0; c->P.limited = beta > 0.0 ? 1 : 0;
+    c->min_valid = false;
+    k_reset_min<<<1, 1, 0, c->stream>>>(c->d_S);
+    return SWE_OK;
+}
+
+int swe_set_manning(swe_ctx* c, const double* n_cell) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    const int64_t nt = c->H.nt;
+    if (!n_cell) {
+        CU(cudaMemsetAsync(c->g.d_nman, 0, nt * sizeof(double), c->stream));
+    } else {
+        const double* src = n_cell;
+        if (!is_device_ptr(n_cell)) {
+            int rc = ensure_stage(c, (size_t)nt); if (rc) return rc;
+            CU(cudaMemcpyAsync(c->d_stage, n_cell, nt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+            src = c->d_stage;
+        }
+        k_scalar_from_user<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(c->g.d_nman, c->g.d_cell_user, src, (int)nt);
+        CU(cudaGetLastError());
+    }
+    if (c->has_zones) {
+        k_gather_scalar<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.d_nman, c->g.d_nman, c->d_src_of_cell, (int)c->z.nc);
+        CU(cudaGetLastError());
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_set_bc(swe_ctx* c, int tag, int kind, double value) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (tag < 0 || kind < 0 || kind > 3 || value != value) return fail(SWE_ERR_ARG, "bad boundary condition");
+    c->bc[tag] = {kind, value};
+    int rc = refresh_bc(c, c->g);
+    if (rc == SWE_OK && c->has_zones) rc = refresh_bc(c, c->z);
+    return rc;
+}
+
+int swe_set_state(swe_ctx* c, const double* h, const double* hu, const double* hv) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!h || !hu || !hv) return fail(SWE_ERR_ARG, "NULL state array");
+    const int64_t nt = c->H.nt;
+    const double *dh = h, *dhu = hu, *dhv = hv;
+    const bool dev = is_device_ptr(h) && is_device_ptr(hu) && is_device_ptr(hv);
+    if (!dev) {
+        int rc = ensure_stage(c, 3 * (size_t)nt + 2); if (rc) return rc;
+        CU(cudaMemcpyAsync(c->d_stage, h, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(c->d_stage + nt, hu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(c->d_stage + 2 * nt, hv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        dh = c->d_stage; dhu = c->d_stage + nt; dhv = c->d_stage + 2 * nt;
+    }
+    int* flag = nullptr;
+    CU(cudaMalloc((void**)&flag, sizeof(int)));
+    cudaMemsetAsync(flag, 0, sizeof(int), c->stream);
+    k_check_state<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(dh, nt, flag);
+    int bad = 0;
+    cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    cudaFree(flag);
+    if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    if (bad) return fail(SWE_ERR_STATE, "h contains NaN or a negative depth");
+    k_state_from_user<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(c->g.A, c->g.d_cell_user, c->g.dm.zc, dh, dhu, dhv, (int)nt);
+    c->launches += 2;
+    if (c->has_zones) {
+        k_gather_cells<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.A, c->g.A, c->d_src_of_cell, (int)c->z.nc);
+        c->launches++;
+    }
+    k_reset_min<<<1, 1, 0, c->stream>>>(c->d_S);
+    c->min_valid = false;
+    CU(cudaGetLastError());
+    if (!dev) CU(cudaStreamSynchronize(c->stream));   // the staging buffer may be reused
+    return SWE_OK;
+}
+
+int swe_get_state(const swe_ctx* cc, double* h, double* hu, double* hv) {
+    swe_ctx* c = const_cast<swe_ctx*>(cc);
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!h || !hu || !hv) return fail(SWE_ERR_ARG, "NULL state array");
+    const int64_t nt = c->H.nt;
+    const bool dev = is_device_ptr(h) && is_device_ptr(hu) && is_device_ptr(hv);
+    double *dh = h, *dhu = hu, *dhv = hv;
+    if (!dev) {
+        int rc = ensure_stage(c, 3 * (size_t)nt + 2); if (rc) return rc;
+        dh = c->d_stage; dhu = c->d_stage + nt; dhv = c->d_stage + 2 * nt;
+    }
+    Store& st = c->active();
+    k_state_to_user<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.A, st.d_cell_user, st.dm.layer, dh, dhu, dhv, (int)st.nc);
+    c->launches++;
+    CU(cudaGetLastError());
+    if (!dev) {
+        CU(cudaMemcpyAsync(h, dh, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(hu, dhu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(hv, dhv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_set_time(swe_ctx* c, double t) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    CU(cudaMemcpyAsync(&c->d_S->t, &t, sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (nsteps < 0 || !(cfl > 0.0) || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad step arguments");
+    if (c->has_zones && scheme == K_WAF && c->Z.nlayers < 2)
+        return fail(SWE_ERR_STATE, "WAF needs zones with at least 2 ghost layers");
+    Store& st = c->active();
+    for (int s = 0; s < nsteps; ++s) {
+        if (!c->min_valid) run_dt_reduce(c, st, st.A);                      // a9
+        launch(c, KIND_MISC, [&] { k_dt_finalize<<<1, 1, 0, c->stream>>>(c->d_S, cfl, 1); });
+        if (scheme == K_MUSCL) {                                            // Heun RK2 (A.11)
+            run_stage(c, st, st.A, nullptr, st.B, scheme, 0, false);
+            run_stage(c, st, st.B, st.A, st.A, scheme, 1, true);
+        } else {
+            run_stage(c, st, st.A, nullptr, st.A, scheme, 0, true);
+        }
+        c->min_valid = true;
+        c->steps++;
+    }
+    CU(cudaGetLastError());
+    if (c->profile) profile_collect(c);
+    if (t_out || last_dt_out) {
+        StepScalars hs;
+        CU(cudaMemcpyAsync(&hs, c->d_S, sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if (t_out) *t_out = hs.t;
+        if (last_dt_out) *last_dt_out = hs.last_dt;
+    }
+    return SWE_OK;
+}
+
+int swe_step_timed(swe_ctx* c, int nsteps, double cfl, int scheme, float* ms_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    cudaEvent_t a, b;
+    CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
+    CU(cudaEventRecord(a, c->stream));
+    int rc = swe_step(c, nsteps, cfl, scheme, nullptr, nullptr);
+    cudaEventRecord(b, c->stream);
+    cudaError_t e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    if (rc != SWE_OK) return rc;
+    if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    if (ms_out) *ms_out = ms;
+    return SWE_OK;
+}
+
+int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (which < 0 || which > 6 || scheme < 0 || scheme > 2 || reps < 1) return fail(SWE_ERR_ARG, "bad kernel selector");
+    Store& st = c->active();
+    const bool prof = c->profile; c->profile = false;
+    // make the inputs of the timed kernel valid
+    if (scheme == K_MUSCL && which >= 2) run_grad(c, st, st.A);
+    if (which >= 3 && which <= 4) run_flux(c, st, st.A, scheme);
+    cudaEvent_t a, b;
+    CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
+    CU(cudaEventRecord(a, c->stream));
+    for (int r = 0; r < reps; ++r) {
+        switch (which) {
+            case 0: run_dt_reduce(c, st, st.A); break;
+            case 1: run_grad(c, st, st.A); break;
+            case 2: run_flux(c, st, st.A, scheme); break;
+            case 3: run_update(c, st, st.A, nullptr, st.B, 0, false); break;
+            case 4: run_update(c, st, st.B, st.A, st.B, 1, false); break;
+            case 5: if (c->has_zones) run_exchange_state(c, st.A, 0, c->nsend, true, false); break;
+            case 6: if (c->has_zones) run_exchange_state(c, st.A, 0, c->nsend, false, true); break;
+        }
+    }
+    cudaEventRecord(b, c->stream);
+    cudaError_t e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    c->profile = prof;
+    if (which == 0) c->min_valid = true;
+    if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    if (ms_out) *ms_out = ms;
+    return SWE_OK;
+}
+
+int swe_set_profile(swe_ctx* c, int on) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    profile_collect(c);
+    c->profile = on != 0;
+    for (int k = 0; k < NKIND; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    return SWE_OK;
+}
+int swe_get_profile(swe_ctx* c, double* ms /*7*/, int64_t* count /*7*/) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    profile_collect(c);
+    for (int k = 0; k < NKIND; ++k) { if (ms) ms[k] = c->prof_ms[k]; if (count) count[k] = c->prof_n[k]; }
+    return SWE_OK;
+}
+
+int swe_compute_dt(swe_ctx* c, double cfl, double* dt_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!(cfl > 0.0) || !dt_out) return fail(SWE_ERR_ARG, "bad arguments");
+    Store& st = c->active();
+    run_dt_reduce(c, st, st.A);
+    c->min_valid = true;
+    StepScalars hs;
+    CU(cudaMemcpyAsync(&hs, c->d_S, sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    double m;
+    std::memcpy(&m, &hs.min_bits, sizeof(double));
+    *dt_out = std::isinf(m) ? 0.0 : cfl * m;
+    return SWE_OK;
+}
+
+static int out_to_user(swe_ctx* c, double* out, size_t n, double** dev_out) {
+    if (is_device_ptr(out)) { *dev_out = out; return SWE_OK; }
+    int rc = ensure_stage(c, n); if (rc) return rc;
+    *dev_out = c->d_stage;
+    return SWE_OK;
+}
+static int finish_out(swe_ctx* c, double* out, size_t n, double* dev_out) {
+    if (dev_out != out) CU(cudaMemcpyAsync(out, dev_out, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_gradients(swe_ctx* c, double* out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!out) return fail(SWE_ERR_ARG, "NULL output");
+    if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
+    double* d; int rc = out_to_user(c, out, 8 * (size_t)c->g.nc, &d); if (rc) return rc;
+    run_grad(c, c->g, c->g.A);
+    k_grad_to_user<<<grid_for(c->g.nc, c->grid_light), 256, 0, c->stream>>>(c->g.grad, c->g.d_cell_user, d, (int)c->g.nc);
+    CU(cudaGetLastError());
+    return finish_out(c, out, 8 * (size_t)c->g.nc, d);
+}
+
+int swe_side_fluxes(swe_ctx* c, double dt, int scheme, double* out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!out || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad arguments");
+    if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
+    double* d; int rc = out_to_user(c, out, 9 * (size_t)c->g.nc, &d); if (rc) return rc;
+    k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);
+    if (scheme == K_MUSCL) run_grad(c, c->g, c->g.A);
+    run_flux(c, c->g, c->g.A, scheme);
+    k_side_flux_to_user<<<grid_for(c->g.nc, c->grid_light), 256, 0, c->stream>>>(c->g.dm, c->g.F, c->g.d_cell_user, d);
+    CU(cudaGetLastError());
+    return finish_out(c, out, 9 * (size_t)c->g.nc, d);
+}
+
+int swe_euler_stage(swe_ctx* c, double dt, int scheme, double* h1, double* hu1, double* hv1) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!h1 || !hu1 || !hv1 || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad arguments");
+    if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
+    const int64_t nt = c->g.nc;
+    k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);
+    if (scheme == K_MUSCL) run_grad(c, c->g, c->g.A);
+    run_flux(c, c->g, c->g.A, scheme);
+    run_update(c, c->g, c->g.A, nullptr, c->g.B, 0, false);
+    const bool dev = is_device_ptr(h1) && is_device_ptr(hu1) && is_device_ptr(hv1);
+    double *dh = h1, *dhu = hu1, *dhv = hv1;
+    if (!dev) {
+        int rc = ensure_stage(c, 3 * (size_t)nt + 2); if (rc) return rc;
+        dh = c->d_stage; dhu = c->d_stage + nt; dhv = c->d_stage + 2 * nt;
+    }
+    k_state_to_user<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(c->g.B, c->g.d_cell_user, nullptr, dh, dhu, dhv, (int)nt);
+    CU(cudaGetLastError());
+    if (!dev) {
+        CU(cudaMemcpyAsync(h1, dh, nt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(hu1, dhu, nt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(hv1, dhv, nt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_get_stats(const swe_ctx* c, int64_t* steps, int64_t* kernel_launches, int64_t* halo_bytes) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (steps) *steps = c->steps;
+    if (kernel_launches) *kernel_launches = c->launches;
+    if (halo_bytes) *halo_bytes = c->halo_bytes;
+    return SWE_OK;
+}
+
+// ---- zones ----
+int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (nzones < 0) return fail(SWE_ERR_ARG, "nzones must be >= 0");
+    int rc = sync_global_from_zoned(c); if (rc) return rc;
+    CU(cudaStreamSynchronize(c->stream));
+    free_zones(c);
+    c->min_valid = false;
+    k_reset_min<<<1, 1, 0, c->stream>>>(c->d_S);
+    if (nzones == 0) return SWE_OK;
+    std::vector<int32_t> hz;
+    if (zone_of_cell && is_device_ptr(zone_of_cell)) {
+        hz.resize(c->H.nt);
+        CU(cudaMemcpy(hz.data(), zone_of_cell, c->H.nt * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        zone_of_cell = hz.data();
+    }
+    std::string err;
+    bool ok = false;
+    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err); }
+    catch (const std::bad_alloc&) { c->Z = ZoneSet(); return fail(SWE_ERR_NOMEM, "out of host memory in zone set-up"); }
+    if (!ok) { c->Z = ZoneSet(); return fail(SWE_ERR_ARG, err); }
+    rc = upload_store(c, c->z, c->Z.mesh);
+    if (rc) { free_zones(c); return rc; }
+    c->z.dm.glayer = (nlayers >= 2) ? 1 : 0;
+    {   // ghost layer per cell as bytes
+        std::vector<uint8_t> lay((size_t)c->z.nc);
+        for (int64_t i = 0; i < c->z.nc; ++i) lay[i] = (uint8_t)c->Z.mesh.c2c[4 * i + 3];
+        uint8_t* d_lay;
+        CU(c->z.upload(&d_lay, lay.data(), lay.size(), c->stream));
+        c->z.dm.layer = d_lay;
+    }
+    c->nsend = (int64_t)c->Z.send_idx.size();
+    const size_t ns = (size_t)(c->nsend ? c->nsend : 1);
+    CU(cudaMalloc((void**)&c->d_send_idx, ns * sizeof(int)));
+    CU(cudaMalloc((void**)&c->d_recv_idx, ns * sizeof(int)));
+    CU(cudaMalloc((void**)&c->d_src_of_cell, (size_t)c->z.nc * sizeof(int)));
+    CU(cudaMalloc((void**)&c->d_sendbuf, ns * 8 * sizeof(double)));
+    if (c->nsend) {
+        CU(cudaMemcpyAsync(c->d_send_idx, c->Z.send_idx.data(), c->nsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_recv_idx, c->Z.recv_idx.data(), c->nsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    }
+    CU(cudaMemcpyAsync(c->d_src_of_cell, c->Z.src_of_cell.data(), (size_t)c->z.nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    c->has_zones = true;
+    rc = refresh_bc(c, c->z); if (rc) return rc;
+    k_gather_cells<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.A, c->g.A, c->d_src_of_cell, (int)c->z.nc);
+    k_gather_cells<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.B, c->g.A, c->d_src_of_cell, (int)c->z.nc);
+    k_gather_scalar<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.d_nman, c->g.d_nman, c->d_src_of_cell, (int)c->z.nc);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(c->stream));
+    // the host copies of the big zoned arrays are no longer needed
+    c->Z.mesh = MeshArrays();
+    return SWE_OK;
+}
+
+static int exchange_zone(swe_ctx* c, int zone, bool pack) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones: call swe_zones_create first");
+    if (zone < -1 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "zone out of range");
+    if (zone == -1) {
+        run_exchange_state(c, c->z.A, 0, c->nsend, pack, !pack);
+    } else {
+        for (size_t l = 0; l + 1 < c->Z.link_off.size(); ++l) {
+            const int who = pack ? c->Z.link_src[l] : c->Z.link_dst[l];
+            if (who != zone) continue;
+            run_exchange_state(c, c->z.A, c->Z.link_off[l], c->Z.link_off[l + 1] - c->Z.link_off[l], pack, !pack);
+        }
+    }
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+int swe_pack_ghosts(swe_ctx* c, int zone) { return exchange_zone(c, zone, true); }
+int swe_unpack_ghosts(swe_ctx* c, int zone) { return exchange_zone(c, zone, false); }
+
+int swe_zone_stats(const swe_ctx* c, int64_t* send_cells_total, int64_t* bytes_per_exchange, int64_t* ghost_cells_total) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    int64_t gh = 0;
+    for (const ZoneDesc& zd : c->Z.z) gh += (int64_t)zd.cells.size() - zd.nowned;
+    if (send_cells_total) *send_cells_total = c->nsend;
+    if (bytes_per_exchange) *bytes_per_exchange = c->nsend * 24;
+    if (ghost_cells_total) *ghost_cells_total = gh;
+    return SWE_OK;
+}
+int swe_zone_describe(const swe_ctx* c, int zone, int64_t* nowned, int64_t* nghost, int64_t* nlinks) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
+    const ZoneDesc& zd = c->Z.z[zone];
+    if (nowned) *nowned = zd.nowned;
+    if (nghost) *nghost = (int64_t)zd.cells.size() - zd.nowned;
+    if (nlinks) *nlinks = (int64_t)zd.links.size();
+    return SWE_OK;
+}
+int swe_zone_cells(const swe_ctx* c, int zone, int32_t* cells, int32_t* layer) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
+    const ZoneDesc& zd = c->Z.z[zone];
+    for (size_t j = 0; j < zd.cells.size(); ++j) {
+        if (cells) cells[j] = c->H.m.cell_user[zd.cells[j]];
+        if (layer) layer[j] = zd.layer[j];
+    }
+    return SWE_OK;
+}
+int swe_zone_links(const swe_ctx* c, int zone, int32_t* src, int32_t* start, int32_t* count) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
+    const ZoneDesc& zd = c->Z.z[zone];
+    for (size_t j = 0; j < zd.links.size(); ++j) {
+        if (src) src[j] = zd.links[j].src;
+        if (start) start[j] = zd.links[j].start;
+        if (count) count[j] = zd.links[j].count;
+    }
+    return SWE_OK;
+}
+int swe_zone_sendlist(const swe_ctx* c, int zone, int link, int32_t* send_idx) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
+    const ZoneDesc& zd = c->Z.z[zone];
+    if (link < 0 || link >= (int)zd.links.size() || !send_idx) return fail(SWE_ERR_ARG, "no such link");
+    std::copy(zd.links[link].send.begin(), zd.links[link].send.end(), send_idx);
+    return SWE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,298 @@
+"""GPU parity tests proper: the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): max relative error <= 1e-11 per step,
+<= 1e-8 after the stated step counts, identical wet/dry masks."""
+import numpy as np
+import pytest
+
+import paper_2307_16758_b200 as sw
+from oracle import pyoracle as po
+from swe_inputs import config0, config1, config2, config3, lake_case, simple_wave_case
+from parity import assert_parity, rel_errors
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-11
+TOL_RUN = 1e-8
+
+
+@pytest.fixture(autouse=True)
+def _threads():
+    po.set_threads(0)
+
+
+def _pair(cfg, renumber=sw.SWE_RENUM_HILBERT):
+    return po.Oracle.from_config(cfg), sw.create_from_config(cfg, renumber)
+
+
+def _small_cases():
+    river = config3(length=3200.0, half_width=600.0, w2=30.0, n4=4, n8=3)
+    ritter = config0(nx=100, ny=6, h_right=0.0)
+    wave = simple_wave_case(120, jitter=0.1)
+    c1 = config1(n=48)
+    lake = lake_case(n=40)
+    return {"c0": config0(), "ritter": ritter, "wave": wave, "c1": c1, "lake": lake, "river": river}
+
+
+# ---------------------------------------------------------------------------------------------
+# single passes (rows a2, a3-a7, a8, a9 of the scope table)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c0", "ritter", "c1", "lake", "river"])
+def test_single_passes_match_oracle(name):
+    cfg = _small_cases()[name]
+    o, c = _pair(cfg)
+    try:
+        # move away from the initial state so that every field is non-trivial
+        scheme0, cfl0, _ = cfg["runs"][0]
+        o.step(7, cfl0, scheme0)
+        sw.swe_set_state(c, *o.get_state())
+        for cfl in (0.9, 0.45):
+            dt_o = o.compute_dt(cfl)
+            dt_g = sw.swe_compute_dt(c, cfl)
+            assert abs(dt_g - dt_o) <= 4e-16 * dt_o
+        dt = o.compute_dt(0.45)
+        # a2 gradients
+        go = o.gradients()
+        gg = sw.swe_gradients(c)
+        for q in range(4):
+            sc = max(np.abs(go[:, 2 * q:2 * q + 2]).max(), 1e-300)
+            if name != "lake":
+                assert np.abs(gg[:, 2 * q:2 * q + 2] - go[:, 2 * q:2 * q + 2]).max() <= 1e-11 * max(sc, 1e-3)
+        # a3-a7 fluxes per cell side
+        c2c, c2e = o.cell_topology()
+        eg = o.edge_geometry()
+        edges = np.unique(np.linspace(0, o.ne - 1, 1200).astype(np.int64))
+        for scheme in ("hllc", "muscl", "waf"):
+            fg = sw.swe_side_fluxes(c, dt, scheme)
+            got, ref = [], []
+            for e in edges:
+                a, b = o.edge_flux(int(e), dt, scheme)
+                L, R = eg["eL"][e], eg["eR"][e]
+                got.append(fg[L, int(np.nonzero(c2e[L] == e)[0][0])]); ref.append(a)
+                if R >= 0:
+                    got.append(fg[R, int(np.nonzero(c2e[R] == e)[0][0])]); ref.append(-b)
+            got, ref = np.array(got), np.array(ref)
+            sc = max(np.abs(ref).max(), 1e-300)
+            assert np.abs(got - ref).max() <= 1e-11 * sc, (scheme, np.abs(got - ref).max(), sc)
+            # a8 one Euler stage
+            ho = o.euler_stage(dt, scheme)
+            hg = sw.swe_euler_stage(c, dt, scheme)
+            assert_parity(ho, hg, TOL_STEP, what="%s %s stage" % (name, scheme))
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+@pytest.mark.parametrize("name", ["c0", "ritter", "wave", "c1", "lake", "river"])
+@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45)])
+def test_per_step_and_run_parity_small(name, scheme, cfl):
+    """Per step: both sides start every step from the oracle's state (<= 1e-11).  Then a free run
+    of the same length from the initial state (<= 1e-8)."""
+    cfg = _small_cases()[name]
+    o, c = _pair(cfg)
+    nsteps = 60
+    try:
+        worst = 0.0
+        for s in range(nsteps):
+            sw.swe_set_state(c, *o.get_state())
+            to, dto = o.step(1, cfl, scheme)
+            tg, dtg = sw.swe_step(c, 1, cfl, scheme)
+            assert abs(dtg - dto) <= 4e-16 * max(dto, 1e-300)
+            e = assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="%s %s step %d" % (name, scheme, s))
+            worst = max(worst, max(e.values()))
+        o2, c2 = _pair(cfg, sw.SWE_RENUM_NONE)
+        try:
+            o2.step(nsteps, cfl, scheme)
+            t, _ = sw.swe_step(c2, nsteps, cfl, scheme)
+            assert_parity(o2.get_state(), sw.swe_get_state(c2), TOL_RUN, what="%s %s run" % (name, scheme))
+        finally:
+            sw.swe_mesh_destroy(c2)
+            o2.close()
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+def test_renumbering_is_invisible():
+    """Hilbert and identity numbering give bit-identical results (orientation, summation order and
+    dt do not depend on the internal numbering)."""
+    cfg = _small_cases()["river"]
+    a = sw.create_from_config(cfg, sw.SWE_RENUM_NONE)
+    b = sw.create_from_config(cfg, sw.SWE_RENUM_HILBERT)
+    try:
+        for scheme, cfl in (("muscl", 0.45), ("waf", 0.45), ("hllc", 0.9)):
+            ta = sw.swe_step(a, 25, cfl, scheme)
+            tb = sw.swe_step(b, 25, cfl, scheme)
+            assert ta == tb
+            for x, y in zip(sw.swe_get_state(a), sw.swe_get_state(b)):
+                assert np.array_equal(x, y)
+    finally:
+        sw.swe_mesh_destroy(a)
+        sw.swe_mesh_destroy(b)
+
+
+# ---------------------------------------------------------------------------------------------
+# the BASELINE.json configs at full size
+# ---------------------------------------------------------------------------------------------
+def test_config0_full():
+    """configs[0]: 4 000 cells, HLLC, CFL 0.9, 200 steps: per-step and end-of-run parity."""
+    cfg = config0()
+    o, c = _pair(cfg)
+    try:
+        for s in range(200):
+            sw.swe_set_state(c, *o.get_state())
+            o.step(1, 0.9, "hllc")
+            sw.swe_step(c, 1, 0.9, "hllc")
+            assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c0 step %d" % s)
+        sw.swe_set_state(c, cfg["h"], cfg["hu"], cfg["hv"])
+        sw.swe_set_time(c, 0.0)
+        tg, _ = sw.swe_step(c, 200, 0.9, "hllc")
+        assert abs(tg - o.step(0, 0.9, "hllc")[0]) <= 1e-12 * tg
+        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_RUN, what="c0 run")
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+def test_config1_full():
+    """configs[1]: 245 000 cells in random order, MUSCL (beta=1) Heun RK2, CFL 0.45, 500 steps."""
+    cfg = config1()
+    o, c = _pair(cfg)
+    try:
+        area = o.cell_geometry()["area"]
+        m0 = float(np.sum(cfg["h"] * area))
+        done = 0
+        for chunk in (1, 9, 90, 400):
+            o.step(chunk, 0.45, "muscl")
+            sw.swe_step(c, chunk, 0.45, "muscl")
+            done += chunk
+            tol = TOL_STEP if done == 1 else TOL_RUN
+            assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c1 after %d steps" % done)
+        h, hu, hv = sw.swe_get_state(c)
+        assert abs(float(np.sum(h * area)) - m0) <= 1e-12 * m0           # mass, wall boundaries
+        assert h.min() >= 1.0 - 1e-9 and h.max() <= 10.0 + 1e-9
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+@pytest.mark.parametrize("scheme", ["waf", "muscl"])
+def test_config2_full(scheme):
+    """configs[2]: ~1.0 M cells, lake at rest over rough bathymetry with dry bump tops, Manning
+    0.03, 1 000 steps: velocity <= 1e-12, mass conserved, masks identical; oracle parity over the
+    first 100 steps (the oracle needs minutes for 1 000) and GPU-only invariants to step 1 000."""
+    cfg = config2()
+    o, c = _pair(cfg)
+    try:
+        area = o.cell_geometry()["area"]
+        m0 = float(np.sum(cfg["h"] * area))
+        wet0 = cfg["h"] > 1e-6
+        o.step(1, 0.45, scheme)
+        sw.swe_step(c, 1, 0.45, scheme)
+        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c2 %s step 1" % scheme)
+        o.step(99, 0.45, scheme)
+        sw.swe_step(c, 99, 0.45, scheme)
+        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_RUN, what="c2 %s 100 steps" % scheme)
+        sw.swe_step(c, 900, 0.45, scheme)
+        h, hu, hv = sw.swe_get_state(c)
+        wet = h > 1e-6
+        assert np.array_equal(wet, wet0)
+        vel = np.sqrt(hu[wet] ** 2 + hv[wet] ** 2) / h[wet]
+        assert vel.max() <= 1e-12, vel.max()
+        assert abs(float(np.sum(h * area)) - m0) <= 1e-13 * m0
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+def test_config3_reduced_long_run():
+    """configs[3] structure at reduced size (same generator: banded river mesh, inflow Q, fixed
+    level, partly dry, Manning by zone), 200 steps MUSCL and HLLC; inflow volume balance."""
+    cfg = config3(length=6400.0, half_width=1000.0, w2=40.0, n4=6, n8=4)
+    for scheme, cfl in (("muscl", 0.45), ("hllc", 0.9)):
+        o, c = _pair(cfg)
+        try:
+            o.step(1, cfl, scheme)
+            sw.swe_step(c, 1, cfl, scheme)
+            assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c3r %s step 1" % scheme)
+            to, _ = o.step(199, cfl, scheme)
+            tg, _ = sw.swe_step(c, 199, cfl, scheme)
+            assert abs(tg - to) <= 1e-11 * to
+            assert_parity(o.get_state(), sw.swe_get_state(c), TOL_RUN, what="c3r %s 200 steps" % scheme)
+        finally:
+            sw.swe_mesh_destroy(c)
+            o.close()
+
+
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9)])
+def test_config3_full_first_steps(scheme, cfl):
+    """configs[3] at full size (~13 M cells), in the launch configuration bench.py times: the
+    oracle advances 2 steps (it needs ~10 s per step), compared element by element."""
+    cfg = config3()
+    o, c = _pair(cfg)
+    try:
+        assert o.nt > 12_000_000
+        o.step(1, cfl, scheme)
+        sw.swe_step(c, 1, cfl, scheme)
+        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c3 %s step 1" % scheme)
+        o.step(1, cfl, scheme)
+        sw.swe_step(c, 1, cfl, scheme)
+        assert_parity(o.get_state(), sw.swe_get_state(c), 10 * TOL_STEP, what="c3 %s step 2" % scheme)
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------
+def test_edge_cases():
+    # a single triangle, all walls: nothing moves
+    x = np.array([0.0, 1.0, 0.0]); y = np.array([0.0, 0.0, 1.0]); z = np.zeros(3)
+    c = sw.swe_mesh_create(x, y, z, np.array([[0, 1, 2]], np.int32))
+    try:
+        sw.swe_set_state(c, np.array([2.0]), np.array([0.0]), np.array([0.0]))
+        for scheme in ("hllc", "muscl", "waf"):
+            sw.swe_step(c, 5, 0.45, scheme)
+        h, hu, hv = sw.swe_get_state(c)
+        assert h[0] == 2.0 and abs(hu[0]) <= 1e-15 and abs(hv[0]) <= 1e-15
+        # all dry: dt = 0 and the step is a no-op (A.2)
+        sw.swe_set_state(c, np.zeros(1), np.zeros(1), np.zeros(1))
+        t0, _ = sw.swe_step(c, 0, 0.9, "hllc")
+        t1, dt = sw.swe_step(c, 3, 0.9, "hllc")
+        assert dt == 0.0 and t1 == t0
+        assert sw.swe_compute_dt(c, 0.9) == 0.0
+        # bad state
+        with pytest.raises(sw.SweError) as e:
+            sw.swe_set_state(c, np.array([-1.0]), np.zeros(1), np.zeros(1))
+        assert e.value.code == sw.SWE_ERR_STATE
+        with pytest.raises(sw.SweError):
+            sw.swe_set_state(c, np.array([np.nan]), np.zeros(1), np.zeros(1))
+        with pytest.raises(sw.SweError):
+            sw.swe_step(c, 1, -1.0, "hllc")
+        with pytest.raises(sw.SweError):
+            sw.swe_step(c, 1, 0.5, 7)
+    finally:
+        sw.swe_mesh_destroy(c)
+
+
+def test_device_pointers_and_streams():
+    """Arrays may live on the device (torch tensors passed straight through) and the context runs
+    on the caller's stream."""
+    import torch
+    cfg = _small_cases()["c1"]
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        c = sw.create_from_config(cfg, cuda_stream=st.cuda_stream)
+        ref = sw.create_from_config(cfg)
+        try:
+            h = torch.tensor(cfg["h"], device="cuda"); hu = torch.zeros_like(h); hv = torch.zeros_like(h)
+            sw.swe_set_state(c, h, hu, hv)
+            sw.swe_step(c, 10, 0.45, "muscl", sync=False)
+            oh, ohu, ohv = torch.empty_like(h), torch.empty_like(h), torch.empty_like(h)
+            sw.swe_get_state(c, oh, ohu, ohv)
+            sw.swe_step(ref, 10, 0.45, "muscl")
+            r = sw.swe_get_state(ref)
+            assert np.array_equal(oh.cpu().numpy(), r[0]) and np.array_equal(ohu.cpu().numpy(), r[1])
+        finally:
+            sw.swe_mesh_destroy(c)
+            sw.swe_mesh_destroy(ref)
