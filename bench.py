@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark: cell-updates/s of the fp64 MUSCL-RK2 step on the ~13 M-cell
+synthetic river mesh (BASELINE.json configs[3]) on B200, with the HBM roofline of its dominant
+kernel, an end-to-end figure through the C ABI with host buffers, and the CPU oracle timed beside
+it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload c3|c3s|c1|c2]
+                    [--scheme muscl|hllc|waf] [--zones Z --layers L]
+
+One "step" = one full time step (CFL min-reduction, both Heun stages: gradient+limiter, edge flux,
+cell update) over every cell of the mesh.  N > 1 (torchrun): one independent replica of the
+workload per GPU ("replicas only": the multi-GPU halo exchange is row f3 of the scope table, not
+built), weak scaling, value = all ranks' cell-updates / max-over-ranks time.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+ALGO_BYTES = {  # algorithmic bytes per cell (N_e = 1.5 N_c)
+    "grad_limit": 156.0, "edge_flux_muscl": 252.0, "edge_flux_hllc": 140.0, "edge_flux_waf": 296.0,
+    "cell_update_stage": 136.0, "cell_update_final": 168.0, "cell_update_euler": 144.0,
+    "step_muscl": 1120.0, "step_hllc": 284.0, "step_waf": 440.0,
+}
+METRIC = "cell-updates/s (fp64 MUSCL-RK2, 13M cells) and achieved HBM GB/s vs ~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def build_workload(name):
+    from swe_inputs import config1, config2, config3
+    if name == "c3":
+        return config3(), "configs[3]: 60 km x 8 km synthetic river mesh, ~13 M triangles, seed 3"
+    if name == "c3s":
+        return config3(length=6000.0), "configs[3] generator on a 6 km reach (~1.3 M triangles), seed 3"
+    if name == "c3t":
+        return config3(length=1600.0, half_width=600.0), "configs[3] generator, tiny reach (smoke)"
+    if name == "c1":
+        return config1(), "configs[1]: circular dam break, 245 000 triangles, seed 1"
+    if name == "c2":
+        return config2(), "configs[2]: lake at rest, ~1.0 M triangles, seed 2"
+    raise ValueError(name)
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [s.strip() for s in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def traffic_table():
+    """ncu dram bytes per launch (profiles/*.csv written from ncu --set full captures), if any."""
+    out = {}
+    p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if os.path.exists(p):
+        for ln in open(p):
+            f = ln.strip().split(",")
+            if len(f) >= 3 and f[0] != "workload":
+                try:
+                    out[(f[0], f[1])] = float(f[2])
+                except ValueError:
+                    pass
+    return out
+
+
+def oracle_run(cfg, scheme, cfl, warmup, steps):
+    """Times the CPU oracle as it stands (all host cores); returns cell-updates/s and details."""
+    from oracle import pyoracle as po
+    cores = po.set_threads(0)
+    o = po.Oracle.from_config(cfg)
+    if warmup:
+        o.step(warmup, cfl, scheme)
+    t0 = time.perf_counter()
+    o.step(steps, cfl, scheme)
+    dt = time.perf_counter() - t0
+    nt = o.nt
+    o.close()
+    return nt * steps / dt, cores, nt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores, on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sample = "c3s" if args.workload == "c3" else args.workload
+    cfg, desc = build_workload(sample)
+    cfl = 0.9 if args.scheme == "hllc" else 0.45
+    steps = min(args.steps, 8)
+    warm = min(args.warmup, 1)
+    v, cores, nt, secs = oracle_run(cfg, args.scheme, cfl, warm, steps)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "cell-updates/s", "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc, "cells": nt, "scheme": args.scheme, "cfl": cfl},
+        "cpu_baseline": {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle",
+                         "sample": "%s, %d cells, %d steps of %d requested" % (desc, nt, steps, args.steps)},
+        "e2e": {"value": v, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3s", "c3t", "c1", "c2"])
+    ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf"])
+    ap.add_argument("--zones", type=int, default=0)
+    ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2307_16758_b200 import dist as swdist
+    import paper_2307_16758_b200 as sw
+
+    rank, world, local = swdist.init_from_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    sw.lib()   # fails loudly if the CUDA extension is missing
+
+    cfg, desc = build_workload(args.workload)
+    cfl = 0.9 if args.scheme == "hllc" else 0.45
+    ctx = sw.create_from_config(cfg)
+    info = sw.swe_mesh_info(ctx)
+    nt = info["ncell"]
+    if args.zones > 0:
+        sw.swe_zones_create(ctx, args.zones, args.layers)
+
+    # ---- device-resident throughput: warm-up, then exactly K timed steps ----
+    sw.swe_step(ctx, args.warmup, cfl, args.scheme)
+    torch.cuda.synchronize()
+    swdist.barrier()
+    l0 = sw.swe_get_stats(ctx)
+    clk = ClockSampler(local)
+    clk.start()
+    ms = sw.swe_step_timed(ctx, args.steps, cfl, args.scheme)     # CUDA events on the context's stream
+    torch.cuda.synchronize()
+    l1 = sw.swe_get_stats(ctx)
+    swdist.barrier()
+    ms_max = swdist.reduce_max(ms)
+    cells_total = swdist.reduce_sum(float(nt))
+    value = cells_total * args.steps / (ms_max * 1e-3)
+
+    # ---- the same timed region again with per-kernel CUDA events (roofline of the dominant kernel) ----
+    sw.swe_set_profile(ctx, True)
+    sw.swe_step(ctx, args.steps, cfl, args.scheme)
+    prof = sw.swe_get_profile(ctx)
+    sw.swe_set_profile(ctx, False)
+    clocks = clk.stop()
+    peak, peak_src = hbm_peak()
+    kern = {}
+    tot_ms = sum(v[0] for v in prof.values())
+    for k, (kms, n) in prof.items():
+        if n:
+            kern[k] = {"ms_per_launch": kms / n, "launches_per_step": n / args.steps, "share": kms / tot_ms}
+    # algorithmic bytes per launch of each kernel kind (averaged over its launches in a step)
+    if args.scheme == "muscl":
+        algo = {"grad_limit": ALGO_BYTES["grad_limit"], "edge_flux": ALGO_BYTES["edge_flux_muscl"],
+                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
+    elif args.scheme == "hllc":
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_hllc"], "cell_update": ALGO_BYTES["cell_update_euler"]}
+    else:
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_waf"], "cell_update": ALGO_BYTES["cell_update_euler"]}
+    for k in algo:
+        if k in kern:
+            kern[k]["algo_GBps"] = algo[k] * nt / (kern[k]["ms_per_launch"] * 1e-3) / 1e9
+            kern[k]["frac_of_peak"] = kern[k]["algo_GBps"] / peak
+    dom = max((k for k in algo if k in kern), key=lambda k: kern[k]["share"])
+    tt = traffic_table()
+    traffic = tt.get((args.workload, dom + "_" + args.scheme), tt.get((args.workload, dom)))
+    step_bytes = ALGO_BYTES["step_" + args.scheme]
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": kern[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
+        "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+        "algo_bytes_per_launch": algo[dom] * nt,
+        "step_algo_GBps": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9,
+        "step_frac_of_peak": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9 / peak,
+        "step_frac_of_8TBps": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9 / 8000.0,
+        "kernels": kern,
+    }
+
+    # ---- end to end through the C ABI with HOST buffers: every step copies the state host->device
+    # (pinned memory), advances one step and reads the state back ----
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    hbuf = [torch.empty(nt, dtype=torch.float64).pin_memory() for _ in range(3)]
+    sw.swe_get_state(ctx, *hbuf)
+    for _ in range(2):
+        sw.swe_set_state(ctx, *hbuf); sw.swe_step(ctx, 1, cfl, args.scheme, sync=False); sw.swe_get_state(ctx, *hbuf)
+    torch.cuda.synchronize()
+    swdist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sw.swe_set_state(ctx, *hbuf)
+        sw.swe_step(ctx, 1, cfl, args.scheme, sync=False)
+        sw.swe_get_state(ctx, *hbuf)
+    torch.cuda.synchronize()
+    e2e_s = swdist.reduce_max(time.perf_counter() - t0)
+    e2e = {"value": cells_total * e2e_steps / e2e_s, "unit": "cell-updates/s", "steps": e2e_steps,
+           "h2d_bytes_per_step": 3 * 8 * nt, "d2h_bytes_per_step": 3 * 8 * nt,
+           "what": "per step: swe_set_state(pinned host) + swe_step(1) + swe_get_state(pinned host)"}
+    zstats = sw.swe_zone_stats(ctx) if args.zones > 0 else None
+    sw.swe_mesh_destroy(ctx)
+
+    # ---- the oracle as it stands, timed on this box's host cores (rank 0, N=1 only) ----
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sname = "c3s" if args.workload == "c3" else args.workload
+        scfg, sdesc = (cfg, desc) if sname == args.workload else build_workload(sname)
+        osteps = 4
+        v, cores, ont, secs = oracle_run(scfg, args.scheme, cfl, 0, osteps)
+        cpu_baseline = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle",
+                        "sample": "%s: %d cells x %d %s steps in %.1f s" % (sdesc, ont, osteps, args.scheme, secs)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "cell-updates/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "cells": nt, "edges": info["nedge"], "scheme": args.scheme, "cfl": cfl,
+                       "l2": "inputs larger than L2 (state+geometry+flux > 3 GB per stage at 13 M cells)"
+                       if nt > 2_000_000 else "working set may fit L2 at this size",
+                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
+                       "zones": args.zones, "ghost_layers": args.layers if args.zones else 0},
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
+            "gpu_launches": l1["kernel_launches"] - l0["kernel_launches"], "clocks": clocks,
+        }
+        if zstats:
+            line["config"]["zone_stats"] = zstats
+        print(json.dumps(line))
+    swdist.finalize()
+
+
+if __name__ == "__main__":
+    main()
