@@ -69,7 +69,7 @@ struct swe_ctx {
     ZoneSet Z;
     bool has_zones = false;
     Store g, z;
-    Par P{9.81, 1e-6, 1e-3, 0.5, 1};
+    Par P{9.81, 1e-6, 1e-3, 0.5, 1.0 / 9.81, 1};
     double beta = 1.0;
     std::map<int, std::pair<int, double>> bc;
     StepScalars* d_S = nullptr;
@@ -430,7 +430,7 @@ int swe_set_params(swe_ctx* c, double g, double h_dry, double h_thin, double bet
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!(g > 0.0) || !(h_dry >= 0.0) || !(h_thin >= 0.0) || beta != beta) return fail(SWE_ERR_ARG, "bad parameter value");
     c->P.g = g; c->P.h_dry = h_dry; c->P.h_thin = h_thin; c->beta = beta;
-    c->P.kappa = beta / 2.0; c->P.limited = beta > 0.0 ? 1 : 0;
+    c->P.kappa = beta / 2.0; c->P.inv_g = 1.0 / g; c->P.limited = beta > 0.0 ? 1 : 0;
     c->min_valid = false;
     k_reset_min<<<1, 1, 0, c->stream>>>(c->d_S);
     return SWE_OK;
