@@ -14,13 +14,17 @@ SRCS = ["swe_api.cu", "host_mesh.cpp", "host_inspect.cpp"]
 DEPS = SRCS + ["swe_kernels.cuh", "host_mesh.hpp", os.path.join("..", "..", "include", "swe_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+EXTRA = os.environ.get("SWE_NVCC_EXTRA", "").split()   # e.g. -DSWE_FLUX_MINB=4 for tuning sweeps
 
 
 def needs_build():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+    deps = [os.path.join(CSRC, d) for d in DEPS]
+    if not all(os.path.exists(d) for d in deps):
+        return False                      # binary-only copy of the package: use the library as it is
+    return any(os.path.getmtime(d) > t for d in deps)
 
 
 def build(force=False, verbose=False):
@@ -32,7 +36,7 @@ def build(force=False, verbose=False):
              os.path.join(CSRC, n + ".cpp"), "-o", o]
             for n, o in zip(("host_mesh", "host_inspect"), objs)]
     cmds.append([NVCC] + ARCH + ["-lineinfo", "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",
-                                 "-Xptxas", "-v" if verbose else "-O3",
+                                 "-Xptxas", "-v" if verbose else "-O3"] + EXTRA + [
                                  os.path.join(CSRC, "swe_api.cu")] + objs + ["-o", tmp, "-lcudart"])
     try:
         for cmd in cmds:
