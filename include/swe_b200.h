@@ -134,16 +134,14 @@ int swe_get_stats(const swe_ctx* ctx, int64_t* steps, int64_t* kernel_launches, 
 int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_out);
 /* per-kernel timing: runs `reps` launches of one kernel of the hot path on the current state
  * between two events; which: 0 dt_reduce, 1 grad_limit, 2 edge_flux(scheme), 3 cell_update (Euler
- * stage), 4 cell_update (Heun combine), 5 pack, 6 unpack, 7 fused flux+update (Euler stage),
- * 8 fused flux+update (last stage).  The state is left unchanged (updates
+ * stage), 4 cell_update (Heun combine), 5 pack, 6 unpack.  The state is left unchanged (updates
  * write to the stage buffer). */
 int swe_kernel_timed(swe_ctx* ctx, int which, int scheme, int reps, float* ms_out);
 
 /* per-kernel timing inside swe_step: with profiling on, every kernel launch of swe_step is
  * bracketed by two CUDA events on the context's stream; swe_get_profile synchronises and returns
- * accumulated milliseconds and launch counts per kind (8 each):
- * 0 dt_reduce, 1 grad_limit, 2 edge_flux, 3 cell_update, 4 pack, 5 unpack, 6 dt_finalize,
- * 7 flux_update_tile (the fused edge-flux + cell-update kernel). */
+ * accumulated milliseconds and launch counts per kind (7 each):
+ * 0 dt_reduce, 1 grad_limit, 2 edge_flux, 3 cell_update, 4 pack, 5 unpack, 6 dt_finalize. */
 int swe_set_profile(swe_ctx* ctx, int on);
 int swe_get_profile(swe_ctx* ctx, double* ms, int64_t* count);
 

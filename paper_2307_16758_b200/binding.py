@@ -20,8 +20,7 @@ SWE_RENUM_NONE, SWE_RENUM_HILBERT = 0, 1
 SCHEMES = {"hllc": SWE_HLLC, "muscl": SWE_MUSCL, "waf": SWE_WAF}
 BC_KINDS = {"wall": SWE_BC_WALL, "inflow": SWE_BC_INFLOW_Q, "level": SWE_BC_LEVEL,
             "transmissive": SWE_BC_TRANSMISSIVE}
-KERNEL_KINDS = ("dt_reduce", "grad_limit", "edge_flux", "cell_update", "pack", "unpack", "dt_finalize",
-                "flux_update_tile")
+KERNEL_KINDS = ("dt_reduce", "grad_limit", "edge_flux", "cell_update", "pack", "unpack", "dt_finalize")
 
 _lib = None
 _vp, _i64p, _dp = C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_double)
@@ -272,8 +271,8 @@ def swe_set_profile(ctx, on):
 
 
 def swe_get_profile(ctx):
-    ms = (C.c_double * 8)()
-    n = (C.c_int64 * 8)()
+    ms = (C.c_double * 7)()
+    n = (C.c_int64 * 7)()
     _check(lib().swe_get_profile(ctx, ms, n))
     return {k: (ms[i], n[i]) for i, k in enumerate(KERNEL_KINDS)}
 

@@ -280,48 +280,6 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// tiles for the fused flux + update kernel
-// ---------------------------------------------------------------------------------------------
-void build_tiles(const MeshArrays& M, int C, TileArrays& T) {
-    T = TileArrays();
-    T.C = C;
-    T.ntiles = (int)((M.nc + C - 1) / C);
-    T.eoff.assign(T.ntiles + 1, 0);
-    T.eloc.assign(4 * (size_t)M.nc, 0);
-    T.edges.reserve((size_t)(M.ne + M.ne / 8));
-    std::vector<int32_t> stamp(M.ne, -1), slot(M.ne, 0);
-    for (int t = 0; t < T.ntiles; ++t) {
-        const int64_t c0 = (int64_t)t * C, c1 = std::min<int64_t>(M.nc, c0 + C);
-        int n = 0;
-        for (int64_t i = c0; i < c1; ++i) {
-            if (M.c2e[4 * i + 3] != 0) { T.eloc[4 * i + 3] = 0x100; continue; }   // ghost
-            uint16_t flags = 0;
-            for (int k = 0; k < 3; ++k) {
-                const int32_t ce = M.c2e[4 * i + k];
-                const int32_t e = ce >= 0 ? ce : ~ce;
-                if (ce < 0) flags |= (uint16_t)(1u << k);
-                if (stamp[e] != t) { stamp[e] = t; slot[e] = n++; T.edges.push_back(e); }
-                T.eloc[4 * i + k] = (uint16_t)slot[e];
-            }
-            T.eloc[4 * i + 3] = flags;
-        }
-        T.eoff[t + 1] = (int32_t)T.edges.size();
-        T.max_edges = std::max(T.max_edges, n);
-    }
-    const size_t ns = T.edges.size();
-    T.elr.resize(2 * ns); T.en.resize(2 * ns); T.erl.resize(2 * ns); T.err.resize(2 * ns);
-    T.elen.resize(ns); T.edx.resize(ns);
-    for (size_t q = 0; q < ns; ++q) {
-        const size_t e = (size_t)T.edges[q];
-        T.elr[2 * q] = M.elr[2 * e]; T.elr[2 * q + 1] = M.elr[2 * e + 1];
-        T.en[2 * q] = M.en[2 * e]; T.en[2 * q + 1] = M.en[2 * e + 1];
-        T.erl[2 * q] = M.erl[2 * e]; T.erl[2 * q + 1] = M.erl[2 * e + 1];
-        T.err[2 * q] = M.err[2 * e]; T.err[2 * q + 1] = M.err[2 * e + 1];
-        T.elen[q] = M.elen[e]; T.edx[q] = M.edx[e];
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
 // zones (A.12)
 // ---------------------------------------------------------------------------------------------
 namespace {

@@ -31,23 +31,6 @@ struct MeshArrays {
     std::vector<int32_t> btag;               // ne-ne_int: user tag of the boundary edge (-1 = none)
 };
 
-// Tiles of C consecutive cells for the fused flux + update kernel: the distinct edges of the
-// owned cells of each tile (an edge shared by two tiles is listed, and its flux evaluated, in both)
-// and per cell the positions of its three edges in its tile's list.
-struct TileArrays {
-    int C = 0, ntiles = 0, max_edges = 0;
-    std::vector<int32_t> eoff;               // ntiles + 1
-    std::vector<int32_t> edges;              // edge ids, tile after tile
-    // copies of the per-edge arrays in tile order (slot s = eoff[t] + j), so that the fused kernel
-    // streams its edge data instead of gathering it through `edges`
-    std::vector<int32_t> elr;                // 2 per slot
-    std::vector<double> en, erl, err;        // 2 per slot
-    std::vector<double> elen, edx;           // 1 per slot
-    std::vector<uint16_t> eloc;              // 4*nc: slot of side 0,1,2; flags (bit k: cell is the
-                                             //       R-cell of side k; bit 8: ghost cell, no update)
-};
-void build_tiles(const MeshArrays& M, int C, TileArrays& T);
-
 struct ZoneLink {
     int src = -1;
     int32_t start = 0, count = 0;            // receive range, zone-local

@@ -29,7 +29,7 @@ int fail(int code, const std::string& msg) { g_err = msg; return code; }
     } while (0)
 
 enum { KIND_DT = 0, KIND_GRAD = 1, KIND_FLUX = 2, KIND_UPDATE = 3, KIND_PACK = 4, KIND_UNPACK = 5,
-       KIND_MISC = 6, KIND_FUSED = 7, NKIND = 8 };
+       KIND_MISC = 6, NKIND = 7 };
 
 // device copy of one MeshArrays + the state / gradient / flux buffers that live on it
 struct Store {
@@ -42,8 +42,6 @@ struct Store {
     std::vector<int32_t> h_btag;
     double4 *A = nullptr, *B = nullptr, *grad = nullptr;
     FluxBuf F{};
-    TileInfo ti{};                     // tiles of the fused flux + update kernel (C == 0: not built)
-    int grid_tile[3] = {0, 0, 0};      // persistent grid of the fused kernel per scheme
     int64_t nc = 0, ne = 0, nbe = 0;
 
     template <class T> cudaError_t alloc(T** p, size_t n) {
@@ -96,8 +94,6 @@ struct swe_ctx {
     // grid sizes (persistent grid-stride kernels: a multiple of the SM count)
     int grid_light = 148 * 8;
     int grid_grad = 148 * 4, grid_flux[3] = {148 * 4, 148 * 2, 148 * 2}, grid_upd = 148 * 8;
-    int tile_cells = 0;                // cells per tile of the fused flux + update kernel; 0 = three-kernel path
-    int tile_threads = 256;            // threads per block of the fused kernel
 
     Store& active() { return has_zones ? z : g; }
 };
@@ -193,44 +189,6 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.alloc(&st.F.fyl, (size_t)M.ne));
     CU(st.alloc(&st.F.fxr, (size_t)M.ne));
     CU(st.alloc(&st.F.fyr, (size_t)M.ne));
-    if (c->tile_cells > 0) {
-        TileArrays T;
-        build_tiles(M, c->tile_cells, T);
-        int *eoff, *edges; ushort4* eloc;
-        CU(st.upload(&eoff, T.eoff.data(), T.eoff.size(), s));
-        CU(st.upload(&edges, T.edges.data(), T.edges.size(), s));
-        CU(st.upload(&eloc, T.eloc.data(), (size_t)M.nc, s));
-        CU(cudaStreamSynchronize(s));
-        st.ti.C = T.C; st.ti.ntiles = T.ntiles; st.ti.max_edges = T.max_edges;
-        st.ti.eoff = eoff; st.ti.edges = edges; st.ti.eloc = eloc;
-        {
-            int2* telr; double2 *ten, *terl, *terr; double *telen, *tedx;
-            const size_t ns = T.edges.size();
-            CU(st.upload(&telr, T.elr.data(), ns, s));
-            CU(st.upload(&ten, T.en.data(), ns, s));
-            CU(st.upload(&terl, T.erl.data(), ns, s));
-            CU(st.upload(&terr, T.err.data(), ns, s));
-            CU(st.upload(&telen, T.elen.data(), ns, s));
-            CU(st.upload(&tedx, T.edx.data(), ns, s));
-            CU(cudaStreamSynchronize(s));
-            st.ti.g.elr = telr; st.ti.g.en = ten; st.ti.g.erl = terl; st.ti.g.err = terr;
-            st.ti.g.elen = telen; st.ti.g.edx = tedx;
-        }
-        const size_t smem = 5 * (size_t)T.max_edges * sizeof(double);
-        const void* ks[3] = {(const void*)k_flux_update_tile<K_HLLC, 0, true>, (const void*)k_flux_update_tile<K_MUSCL, 1, true>,
-                             (const void*)k_flux_update_tile<K_WAF, 0, true>};
-        const void* all[] = {(const void*)k_flux_update_tile<K_HLLC, 0, true>, (const void*)k_flux_update_tile<K_HLLC, 0, false>,
-                             (const void*)k_flux_update_tile<K_MUSCL, 0, true>, (const void*)k_flux_update_tile<K_MUSCL, 0, false>,
-                             (const void*)k_flux_update_tile<K_MUSCL, 1, true>, (const void*)k_flux_update_tile<K_MUSCL, 1, false>,
-                             (const void*)k_flux_update_tile<K_WAF, 0, true>, (const void*)k_flux_update_tile<K_WAF, 0, false>};
-        if (smem > 48 * 1024)
-            for (const void* k : all) CU(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        for (int q = 0; q < 3; ++q) {
-            int nbk = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, ks[q], c->tile_threads, smem) != cudaSuccess || nbk < 1) { cudaGetLastError(); nbk = 2; }
-            st.grid_tile[q] = nbk * c->num_sm;
-        }
-    }
     CU(cudaMemsetAsync(st.grad, 0, 2 * (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.B, 0, (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.d_nman, 0, (size_t)(M.nc ? M.nc : 1) * sizeof(double), s));
@@ -348,31 +306,6 @@ void run_exchange_grad(swe_ctx* c) {
     c->halo_bytes += count * (4 + 64 + 64 + 4 + 64 + 64);
 }
 
-// fused flux + update over tiles; Uout must not alias Uin
-template <int SCHEME, int MODE, bool FUSE>
-void launch_tile(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout) {
-    const size_t smem = 5 * (size_t)st.ti.max_edges * sizeof(double);
-    int gr = st.grid_tile[SCHEME];
-    if (gr > st.ti.ntiles) gr = st.ti.ntiles;
-    k_flux_update_tile<SCHEME, MODE, FUSE><<<gr, c->tile_threads, smem, c->stream>>>(st.dm, st.ti, Uin, U0, Uout, st.grad, c->P, c->d_S);
-}
-void run_tile(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
-    launch(c, KIND_FUSED, [&] {
-        if (scheme == K_MUSCL) {
-            if (mode == 0 && !fuse) launch_tile<K_MUSCL, 0, false>(c, st, Uin, U0, Uout);
-            else if (mode == 0) launch_tile<K_MUSCL, 0, true>(c, st, Uin, U0, Uout);
-            else if (!fuse) launch_tile<K_MUSCL, 1, false>(c, st, Uin, U0, Uout);
-            else launch_tile<K_MUSCL, 1, true>(c, st, Uin, U0, Uout);
-        } else if (scheme == K_HLLC) {
-            if (fuse) launch_tile<K_HLLC, 0, true>(c, st, Uin, U0, Uout);
-            else launch_tile<K_HLLC, 0, false>(c, st, Uin, U0, Uout);
-        } else {
-            if (fuse) launch_tile<K_WAF, 0, true>(c, st, Uin, U0, Uout);
-            else launch_tile<K_WAF, 0, false>(c, st, Uin, U0, Uout);
-        }
-    });
-}
-
 // one Euler stage on the active store: [exchange] -> [grad (-> exchange grad)] -> flux -> update
 void run_stage(swe_ctx* c, Store& st, double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
     if (c->has_zones) run_exchange_state(c, Uin, 0, c->nsend, true, true);
@@ -380,7 +313,6 @@ void run_stage(swe_ctx* c, Store& st, double4* Uin, const double4* U0, double4* 
         run_grad(c, st, Uin);
         if (c->has_zones && c->Z.nlayers == 1) run_exchange_grad(c);
     }
-    if (st.ti.C > 0 && Uin != Uout) { run_tile(c, st, Uin, U0, Uout, scheme, mode, fuse); return; }
     run_flux(c, st, Uin, scheme);
     run_update(c, st, Uin, U0, Uout, mode, fuse);
 }
@@ -449,11 +381,6 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2);
     c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2);
     c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
-    if (const char* tc = std::getenv("SWE_B200_TILE")) c->tile_cells = std::atoi(tc);
-    if (c->tile_cells < 0 || c->tile_cells > 1024) c->tile_cells = 0;
-    if (c->tile_cells > 256) c->tile_cells = 256;
-    c->tile_threads = ((c->tile_cells + 31) / 32) * 32;                 // one thread per cell of the tile
-    if (c->tile_threads < 32) c->tile_threads = 32;
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
         cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
@@ -622,9 +549,6 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
         if (scheme == K_MUSCL) {                                            // Heun RK2 (A.11)
             run_stage(c, st, st.A, nullptr, st.B, scheme, 0, false);
             run_stage(c, st, st.B, st.A, st.A, scheme, 1, true);
-        } else if (st.ti.C > 0) {                                           // fused kernel: ping-pong
-            run_stage(c, st, st.A, nullptr, st.B, scheme, 0, true);
-            std::swap(st.A, st.B);
         } else {
             run_stage(c, st, st.A, nullptr, st.A, scheme, 0, true);
         }
@@ -662,13 +586,12 @@ int swe_step_timed(swe_ctx* c, int nsteps, double cfl, int scheme, float* ms_out
 
 int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out) {
     if (check_ctx(c)) return SWE_ERR_ARG;
-    if (which < 0 || which > 8 || scheme < 0 || scheme > 2 || reps < 1) return fail(SWE_ERR_ARG, "bad kernel selector");
+    if (which < 0 || which > 6 || scheme < 0 || scheme > 2 || reps < 1) return fail(SWE_ERR_ARG, "bad kernel selector");
     Store& st = c->active();
     const bool prof = c->profile; c->profile = false;
     // make the inputs of the timed kernel valid
     if (scheme == K_MUSCL && which >= 2) run_grad(c, st, st.A);
     if (which >= 3 && which <= 4) run_flux(c, st, st.A, scheme);
-    if (which >= 7 && st.ti.C == 0) return fail(SWE_ERR_STATE, "tiles not built (SWE_B200_TILE)");
     cudaEvent_t a, b;
     CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
     CU(cudaEventRecord(a, c->stream));
@@ -681,8 +604,6 @@ int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out)
             case 4: run_update(c, st, st.B, st.A, st.B, 1, false); break;
             case 5: if (c->has_zones) run_exchange_state(c, st.A, 0, c->nsend, true, false); break;
             case 6: if (c->has_zones) run_exchange_state(c, st.A, 0, c->nsend, false, true); break;
-            case 7: run_tile(c, st, st.A, nullptr, st.B, scheme, 0, false); break;
-            case 8: run_tile(c, st, st.A, st.B, st.B, scheme, scheme == K_MUSCL ? 1 : 0, false); break;
         }
     }
     cudaEventRecord(b, c->stream);
