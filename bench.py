@@ -125,19 +125,22 @@ def traffic_table():
     return out
 
 
-def oracle_run(cfg, scheme, cfl, warmup, steps):
+def oracle_run(cfg, scheme, cfl, warmup, steps, budget_s=None):
     """Times the CPU oracle as it stands (all host cores); returns cell-updates/s and details."""
     from oracle import pyoracle as po
     cores = po.set_threads(0)
     o = po.Oracle.from_config(cfg)
-    if warmup:
-        o.step(warmup, cfl, scheme)
+    t0 = time.perf_counter()
+    o.step(max(1, warmup), cfl, scheme)
+    per = (time.perf_counter() - t0) / max(1, warmup)
+    if budget_s is not None:                      # bounded sample: as many steps as fit the budget
+        steps = int(max(2, min(steps, budget_s / max(per, 1e-9))))
     t0 = time.perf_counter()
     o.step(steps, cfl, scheme)
     dt = time.perf_counter() - t0
     nt = o.nt
     o.close()
-    return nt * steps / dt, cores, nt, dt
+    return nt * steps / dt, cores, nt, dt, steps
 
 
 def run_reference(args):
@@ -148,9 +151,8 @@ def run_reference(args):
     sample = "c3s" if args.workload == "c3" else args.workload
     cfg, desc = build_workload(sample)
     cfl = 0.9 if args.scheme == "hllc" else 0.45
-    steps = min(args.steps, 8)
-    warm = min(args.warmup, 1)
-    v, cores, nt, secs = oracle_run(cfg, args.scheme, cfl, warm, steps)
+    warm = max(1, min(args.warmup, 3))
+    v, cores, nt, secs, steps = oracle_run(cfg, args.scheme, cfl, warm, args.steps, budget_s=90.0)
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": "cell-updates/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": 1e3 * secs / steps, "higher_is_better": True,
@@ -279,8 +281,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sname = "c3s" if args.workload == "c3" else args.workload
         scfg, sdesc = (cfg, desc) if sname == args.workload else build_workload(sname)
-        osteps = 4
-        v, cores, ont, secs = oracle_run(scfg, args.scheme, cfl, 0, osteps)
+        v, cores, ont, secs, osteps = oracle_run(scfg, args.scheme, cfl, 1, 400, budget_s=15.0)
         cpu_baseline = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle",
                         "sample": "%s: %d cells x %d %s steps in %.1f s" % (sdesc, ont, osteps, args.scheme, secs)}
 

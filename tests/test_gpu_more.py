@@ -1,0 +1,147 @@
+"""More GPU parity and API cases: limiter parameter, every boundary kind, parameters changed after
+the mesh / zones exist, launch accounting, per-kernel timing and profiling entry points."""
+import numpy as np
+import pytest
+
+import paper_2307_16758_b200 as sw
+from oracle import pyoracle as po
+from swe_inputs import config0, config3, simple_wave_case, lake_case
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _threads():
+    po.set_threads(0)
+
+
+def _river():
+    return config3(length=3200.0, half_width=600.0, w2=30.0, n4=4, n8=3)
+
+
+@pytest.mark.parametrize("beta", [2.0, 0.0, 1.5])
+def test_limiter_parameter(beta):
+    """beta = 2 (Barth-Jespersen bound), beta <= 0 (unlimited), and a value in between."""
+    cfg = simple_wave_case(120, jitter=0.1)
+    cfg["params"] = dict(cfg["params"], beta=beta)
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        o.step(5, 0.45, "muscl")
+        sw.swe_set_state(c, *o.get_state())
+        go, gg = o.gradients(), sw.swe_gradients(c)
+        assert np.abs(gg - go).max() <= 1e-11 * max(np.abs(go).max(), 1e-3)
+        for s in range(30):
+            sw.swe_set_state(c, *o.get_state())
+            o.step(1, 0.45, "muscl")
+            sw.swe_step(c, 1, 0.45, "muscl")
+            assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="beta %g step %d" % (beta, s))
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+@pytest.mark.parametrize("kinds", [("transmissive", "transmissive"), ("inflow", "transmissive"),
+                                   ("level", "level"), ("wall", "level")])
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45)])
+def test_boundary_kinds(kinds, scheme, cfl):
+    """Every boundary kind (PAPER.md:286 + fixed level) on both tagged boundaries of the river case."""
+    cfg = _river()
+    val = {"transmissive": 0.0, "inflow": 300.0, "level": 3.5, "wall": 0.0}
+    cfg["bc"] = {1: (kinds[0], val[kinds[0]]), 2: (kinds[1], val[kinds[1]])}
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        for s in range(25):
+            sw.swe_set_state(c, *o.get_state())
+            o.step(1, cfl, scheme)
+            sw.swe_step(c, 1, cfl, scheme)
+            assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="%s %s step %d" % (kinds, scheme, s))
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+def test_parameters_changed_after_zones_exist():
+    """swe_set_bc / swe_set_manning / swe_set_params reach the zoned copy as well."""
+    cfg = _river()
+    a = sw.create_from_config(cfg)
+    b = sw.create_from_config(cfg)
+    try:
+        sw.swe_zones_create(b, 8, 2)
+        n2 = np.where(cfg["manning"] > 0.03, 0.05, 0.02)
+        for ctx in (a, b):
+            sw.swe_set_bc(ctx, 1, "inflow", 500.0)
+            sw.swe_set_bc(ctx, 2, "transmissive", 0.0)
+            sw.swe_set_manning(ctx, n2)
+            sw.swe_set_params(ctx, 9.81, 1e-6, 1e-3, 2.0)
+            sw.swe_step(ctx, 20, 0.45, "muscl")
+        for x, y in zip(sw.swe_get_state(a), sw.swe_get_state(b)):
+            assert np.array_equal(x, y)
+        for ctx in (a, b):
+            sw.swe_set_manning(ctx, None)
+            sw.swe_step(ctx, 5, 0.45, "waf")
+        for x, y in zip(sw.swe_get_state(a), sw.swe_get_state(b)):
+            assert np.array_equal(x, y)
+        o = po.Oracle.from_config(cfg)          # and the un-zoned one still matches the oracle
+        o.set_bc(1, "inflow", 500.0); o.set_bc(2, "transmissive", 0.0); o.set_manning(n2)
+        o.set_params(9.81, 1e-6, 1e-3, 2.0)
+        o.step(20, 0.45, "muscl")
+        o.set_manning(None)
+        o.step(5, 0.45, "waf")
+        assert_parity(o.get_state(), sw.swe_get_state(a), 1e-8, what="changed parameters")
+        o.close()
+    finally:
+        sw.swe_mesh_destroy(a)
+        sw.swe_mesh_destroy(b)
+
+
+def test_launch_accounting_and_timing_entry_points():
+    cfg = lake_case(n=40)
+    c = sw.create_from_config(cfg)
+    try:
+        sw.swe_step(c, 1, 0.45, "muscl")                   # includes the stand-alone dt_reduce
+        l0 = sw.swe_get_stats(c)["kernel_launches"]
+        sw.swe_step(c, 10, 0.45, "muscl")
+        l1 = sw.swe_get_stats(c)["kernel_launches"]
+        assert l1 - l0 == 10 * 7                           # finalize + 2 x (grad, flux, update)
+        sw.swe_step(c, 10, 0.9, "hllc")
+        assert sw.swe_get_stats(c)["kernel_launches"] - l1 == 10 * 3
+        assert sw.swe_get_stats(c)["steps"] == 21
+        ms = sw.swe_step_timed(c, 5, 0.45, "muscl")
+        assert ms > 0.0
+        for which in range(5):
+            assert sw.swe_kernel_timed(c, which, "muscl", 3) > 0.0
+        ref = sw.swe_get_state(c)
+        sw.swe_set_profile(c, True)
+        sw.swe_step(c, 4, 0.45, "muscl")
+        p = sw.swe_get_profile(c)
+        sw.swe_set_profile(c, False)
+        assert p["grad_limit"][1] == 8 and p["edge_flux"][1] == 8 and p["cell_update"][1] == 8
+        assert p["dt_finalize"][1] == 4 and p["dt_reduce"][1] == 0
+        assert all(v[0] > 0.0 for k, v in p.items() if v[1])
+        # the timing entry points of single kernels leave the state alone
+        c2 = sw.create_from_config(cfg)
+        sw.swe_step(c2, 1 + 10, 0.45, "muscl"); sw.swe_step(c2, 10, 0.9, "hllc"); sw.swe_step(c2, 5, 0.45, "muscl")
+        for x, y in zip(ref, sw.swe_get_state(c2)):
+            assert np.array_equal(x, y)
+        sw.swe_mesh_destroy(c2)
+    finally:
+        sw.swe_mesh_destroy(c)
+
+
+def test_time_accumulates_and_can_be_set():
+    cfg = config0(nx=60, ny=4)
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        t1, dt1 = sw.swe_step(c, 7, 0.9, "hllc")
+        to, dto = o.step(7, 0.9, "hllc")
+        assert abs(t1 - to) <= 1e-13 * to and abs(dt1 - dto) <= 4e-16 * dto
+        sw.swe_set_time(c, 100.0)
+        t2, dt2 = sw.swe_step(c, 1, 0.9, "hllc")
+        assert abs(t2 - (100.0 + dt2)) <= 1e-12
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
