@@ -10,7 +10,7 @@ import numpy as np
 
 from . import build as _build
 
-SCHEMES = {"hllc": 0, "muscl": 1, "waf": 2}
+SCHEMES = {"hllc": 0, "muscl": 1, "waf": 2, "muscl_ms": 3}
 BC_KINDS = {"wall": 0, "inflow": 1, "level": 2, "transmissive": 3}
 
 _lib = None
@@ -56,6 +56,8 @@ def lib():
         L.orc_waf.argtypes = [C.c_double] * 16 + [C.c_int, _dp]
         L.orc_limiter_A.restype = C.c_double
         L.orc_limiter_A.argtypes = [C.c_double, C.c_double]
+        L.orc_ms_slope.restype = C.c_double
+        L.orc_ms_slope.argtypes = [C.c_double, C.c_double, C.c_double]
         L.orc_manning.argtypes = [C.c_double] * 4 + [_dp, _dp]
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_threads.restype = C.c_int
@@ -97,6 +99,11 @@ def waf(g, h_dry, hL, uL, vL, hR, uR, vR, etaL, etaR, etaLupw, etaRupw, vLupw, v
 
 def limiter_A(r, c):
     return lib().orc_limiter_A(float(r), float(c))
+
+
+def ms_slope(beta, x, y):
+    """Limited slope of the multislope MUSCL, eq. 24-25."""
+    return lib().orc_ms_slope(float(beta), float(x), float(y))
 
 
 def manning(g, n, dt, h, hu, hv):

@@ -17,6 +17,7 @@
 //   eq. 6-14  HLL / HLLC flux, wave speeds
 //   eq. 15-21 WAF flux, TVD weights, SUPERBEE A(r,c)
 //   eq. 24-25 limiter semantics (beta=1 MINBEE) for the cell limiter PAPER.md:410-420
+//   eq. 22-25 the paper's own multislope MUSCL (scheme 3, scope row f1) PAPER.md:396-420
 //   hydrostatic reconstruction, bed-slope and friction sources: named only;
 //   formulas = DESIGN.md readings R12, R15.  LSQ gradients and Heun RK2: BASELINE.json north_star.
 //   zones / ghost layers / send lists / contiguous receive ranges
@@ -45,7 +46,7 @@
 
 namespace {
 
-enum { SCH_HLLC = 0, SCH_MUSCL = 1, SCH_WAF = 2 };
+enum { SCH_HLLC = 0, SCH_MUSCL = 1, SCH_WAF = 2, SCH_MUSCL_MS = 3 };
 enum { BC_WALL = 0, BC_INFLOW = 1, BC_LEVEL = 2, BC_TRANSMISSIVE = 3 };
 
 struct Params {
@@ -68,9 +69,12 @@ struct Mesh {
     std::vector<double> rx, ry;        // 3*nt, r_{i,k} = m_e - c_i
     std::vector<double> nox, noy;      // 3*nt, unit normal of side k outward of cell i
     std::vector<double> wx, wy;        // 3*nt, least-squares weights
+    std::vector<double> dupw;          // 3*nt, |x_i - x_upw| for side k (eq. 22-25): x_upw = mean of the
+                                       // centroids of the two OTHER edge-neighbours (own centroid if missing)
     // per edge
     std::vector<int32_t> eL, eR, ekL, ekR, etag;  // eR=-1, etag=user tag (or -1 = untagged wall)
     std::vector<double> elen, enx, eny, edx;
+    std::vector<double> edlr;          // |x_R - x_L| between the two centroids (0 on the boundary)
 };
 
 struct Ctx {
@@ -215,6 +219,26 @@ bool build_mesh(Mesh& m, int64_t nv, const double* x, const double* y, const dou
             m.wy[3 * i + k] = (-a12 * dxk[k] + a11 * dyk[k]) / det;
         }
     }
+    // distances of the multislope MUSCL (eq. 22-25, reading R17)
+    m.dupw.resize(3 * nt);
+    m.edlr.assign(m.ne, 0.0);
+    for (int64_t i = 0; i < nt; ++i)
+        for (int k = 0; k < 3; ++k) {
+            double sx = 0.0, sy = 0.0;
+            for (int j = 0; j < 3; ++j) {
+                if (j == k) continue;
+                int32_t nb_ = m.c2c[3 * i + j];
+                if (nb_ >= 0) { sx += m.cx[nb_]; sy += m.cy[nb_]; }
+                else { sx += m.cx[i]; sy += m.cy[i]; }
+            }
+            double ux = m.cx[i] - 0.5 * sx, uy = m.cy[i] - 0.5 * sy;
+            m.dupw[3 * i + k] = std::sqrt(ux * ux + uy * uy);
+        }
+    for (int64_t e = 0; e < m.ne; ++e)
+        if (m.eR[e] >= 0) {
+            double ux = m.cx[m.eR[e]] - m.cx[m.eL[e]], uy = m.cy[m.eR[e]] - m.cy[m.eL[e]];
+            m.edlr[e] = std::sqrt(ux * ux + uy * uy);
+        }
     return true;
 }
 
@@ -465,19 +489,64 @@ bool waf_applicable(const Ctx& c, const double* h, int32_t L, int32_t R, double 
 // upwind average over the two other edge-neighbours of cell i; a missing one is
 // replaced by the cell's own value
 void upwind_mean(const Ctx& c, const double* h, const double* hu, const double* hv, int32_t i,
-                 int kskip, const Prim& pi, double& eta, double& u, double& v) {
-    double se = 0.0, su = 0.0, sv = 0.0;
+                 int kskip, const Prim& pi, double& eta, double& u, double& v, double* hmean = nullptr,
+                 bool* all_wet = nullptr) {
+    double se = 0.0, su = 0.0, sv = 0.0, sh = 0.0;
     for (int k = 0; k < 3; ++k) {
         if (k == kskip) continue;
         int32_t nb = c.m.c2c[3 * i + k];
         if (nb >= 0) {
             Prim pk = prim_of(c, h, hu, hv, nb);
-            se += pk.eta; su += pk.u; sv += pk.v;
+            se += pk.eta; su += pk.u; sv += pk.v; sh += pk.h;
+            if (all_wet && !pk.wet) *all_wet = false;
         } else {
-            se += pi.eta; su += pi.u; sv += pi.v;
+            se += pi.eta; su += pi.u; sv += pi.v; sh += pi.h;
         }
     }
     eta = 0.5 * se; u = 0.5 * su; v = 0.5 * sv;
+    if (hmean) *hmean = 0.5 * sh;
+}
+
+// eq. 24-25: limited slope from the slope x on one side and the slope y on the other; the case
+// distinction of the paper is on the sign of y (the printed conditions U_R - U_L > 0 in eq. 24,
+// U_Rupw - U_R > 0 in eq. 25).  beta = 1 MINBEE, beta = 2 SUPERBEE.
+double ms_slope(double beta, double x, double y) {
+    if (y > 0.0) return std::max(0.0, std::max(std::min(beta * x, y), std::min(x, beta * y)));
+    if (y < 0.0) return std::min(0.0, std::min(std::max(beta * x, y), std::max(x, beta * y)));
+    return 0.0;
+}
+
+// eq. 22: face values of the two sides of interior edge e by the multislope reconstruction of
+// q = (eta, h, u, v); first order if a cell of the stencil is not wet (same rule as A.3.5)
+void ms_face_states(const Ctx& c, const double* h, const double* hu, const double* hv, int32_t e,
+                    const Prim& pL, const Prim& pR, Face& fL, Face& fR) {
+    const Mesh& m = c.m;
+    int32_t L = m.eL[e], R = m.eR[e], kL = m.ekL[e], kR = m.ekR[e];
+    fL.eta = pL.eta; fL.h = pL.h; fL.u = pL.u; fL.v = pL.v;
+    fR.eta = pR.eta; fR.h = pR.h; fR.u = pR.u; fR.v = pR.v;
+    bool all_wet = pL.wet && pR.wet;
+    double qLu[4], qRu[4];
+    upwind_mean(c, h, hu, hv, L, kL, pL, qLu[0], qLu[2], qLu[3], &qLu[1], &all_wet);
+    upwind_mean(c, h, hu, hv, R, kR, pR, qRu[0], qRu[2], qRu[3], &qRu[1], &all_wet);
+    if (all_wet) {
+        double beta = c.p.beta > 0.0 ? c.p.beta : 1.0;
+        double dL = m.dupw[3 * L + kL], dR = m.dupw[3 * R + kR], dLR = m.edlr[e];
+        double rL = std::sqrt(m.rx[3 * L + kL] * m.rx[3 * L + kL] + m.ry[3 * L + kL] * m.ry[3 * L + kL]);
+        double rR = std::sqrt(m.rx[3 * R + kR] * m.rx[3 * R + kR] + m.ry[3 * R + kR] * m.ry[3 * R + kR]);
+        double qL[4] = {pL.eta, pL.h, pL.u, pL.v}, qR[4] = {pR.eta, pR.h, pR.u, pR.v};
+        double oL[4], oR[4];
+        for (int q = 0; q < 4; ++q) {
+            double a = (dL > 0.0) ? (qL[q] - qLu[q]) / dL : 0.0;      // upwind slope of L
+            double b = (qR[q] - qL[q]) / dLR;                          // local slope
+            double d = (dR > 0.0) ? (qRu[q] - qR[q]) / dR : 0.0;      // upwind slope of R
+            oL[q] = qL[q] + rL * ms_slope(beta, a, b);                 // eq. 22 with eq. 24
+            oR[q] = qR[q] - rR * ms_slope(beta, b, d);                 // eq. 22 with eq. 25
+        }
+        fL.eta = oL[0]; fL.h = oL[1]; fL.u = oL[2]; fL.v = oL[3];
+        fR.eta = oR[0]; fR.h = oR[1]; fR.u = oR[2]; fR.v = oR[3];
+    }
+    fL.z = fL.eta - fL.h;
+    fR.z = fR.eta - fR.h;
 }
 
 void edge_flux(const Ctx& c, const double* h, const double* hu, const double* hv, const double* grad,
@@ -494,6 +563,10 @@ void edge_flux(const Ctx& c, const double* h, const double* hu, const double* hv
         int32_t kR = m.ekR[e];
         Prim pR = prim_of(c, h, hu, hv, R);
         Face fR = face_state(c, pR, grad, R, kR, scheme);
+        if (scheme == SCH_MUSCL_MS) {
+            ms_face_states(c, h, hu, hv, e, pL, pR, fL, fR);
+            unL = fL.u * n1 + fL.v * n2; utL = -fL.u * n2 + fL.v * n1;
+        }
         double unR = fR.u * n1 + fR.v * n2, utR = -fR.u * n2 + fR.v * n1;
         double zs = std::max(fL.z, fR.z);                               // A.5
         double hsL = std::max(0.0, fL.eta - zs), hsR = std::max(0.0, fR.eta - zs);
@@ -609,7 +682,7 @@ double one_step(Ctx& c, double cfl, int scheme) {
     double dt = compute_dt(c, c.h.data(), c.hu.data(), c.hv.data(), cfl);
     c.a1.resize(nt); c.a2.resize(nt); c.a3.resize(nt);
     if (dt > 0.0) {
-        if (scheme == SCH_MUSCL) {
+        if (scheme == SCH_MUSCL || scheme == SCH_MUSCL_MS) {
             c.b1.resize(nt); c.b2.resize(nt); c.b3.resize(nt);
             euler_stage(c, c.h.data(), c.hu.data(), c.hv.data(), dt, scheme, c.a1.data(), c.a2.data(), c.a3.data());
             euler_stage(c, c.a1.data(), c.a2.data(), c.a3.data(), dt, scheme, c.b1.data(), c.b2.data(), c.b3.data());
@@ -866,7 +939,7 @@ int zones_step(Ctx& c, Zones& Z, double cfl, int scheme) {
         }
     double dt = (best == std::numeric_limits<double>::infinity()) ? 0.0 : cfl * best;
     if (dt > 0.0) {
-        if (scheme == SCH_MUSCL) {
+        if (scheme == SCH_MUSCL || scheme == SCH_MUSCL_MS) {
             for (Zone& zn : Z.z)
                 for (int64_t j = 0; j < zn.nowned; ++j) { zn.h0[j] = zn.h[j]; zn.hu0[j] = zn.hu[j]; zn.hv0[j] = zn.hv[j]; }
             int rc = zones_stage(c, Z, dt, scheme); if (rc) return rc;
@@ -963,7 +1036,7 @@ int orc_get_state(void* p, double* h, double* hu, double* hv) {
 void orc_set_time(void* p, double t) { ((Ctx*)p)->t = t; }
 int orc_step(void* p, int nsteps, double cfl, int scheme, double* t_out, double* dt_out) {
     Ctx* c = (Ctx*)p;
-    if (scheme < 0 || scheme > 2 || nsteps < 0) return -1;
+    if (scheme < 0 || scheme > 3 || nsteps < 0) return -1;
     for (int s = 0; s < nsteps; ++s) one_step(*c, cfl, scheme);
     if (t_out) *t_out = c->t;
     if (dt_out) *dt_out = c->last_dt;
@@ -1040,6 +1113,7 @@ void orc_waf(double g, double h_dry, double hL, double uL, double vL, double hR,
              use_limiter, out);
 }
 double orc_limiter_A(double r, double c) { return limiter_A(r, c); }
+double orc_ms_slope(double beta, double x, double y) { return ms_slope(beta, x, y); }
 void orc_manning(double g, double n, double dt, double h, double* hu, double* hv) {
     manning_step(g, n, dt, h, *hu, *hv);
 }
@@ -1060,7 +1134,7 @@ int orc_zones_step(void* p, int nsteps, double cfl, int scheme, double* t_out, d
     auto it = g_zones.find(c);
     if (it == g_zones.end()) return -4;
     Zones& Z = it->second;
-    int need = (scheme == SCH_HLLC) ? 1 : ((scheme == SCH_WAF) ? 2 : 1);
+    int need = (scheme == SCH_HLLC) ? 1 : ((scheme == SCH_WAF || scheme == SCH_MUSCL_MS) ? 2 : 1);
     if (Z.nlayers < need) return -4;
     for (Zone& zn : Z.z)
         for (int64_t j = 0; j < zn.nowned; ++j) {
