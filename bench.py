@@ -31,6 +31,7 @@ ALGO_BYTES = {  # algorithmic bytes per cell (N_e = 1.5 
     "grad_limit": 156.0, "edge_flux_muscl": 252.0, "edge_flux_hllc": 140.0, "edge_flux_waf": 296.0,
     "cell_update_stage": 136.0, "cell_update_final": 168.0, "cell_update_euler": 144.0,
     "step_muscl": 1120.0, "step_hllc": 284.0, "step_waf": 440.0,
+    "edge_flux_muscl_ms": 200.0, "step_muscl_ms": 704.0,   # 2 x (edge 108 + U 32 + flux 60) + 136 + 168
 }
 METRIC = "cell-updates/s (fp64 MUSCL-RK2, 13M cells) and achieved HBM GB/s vs ~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
@@ -172,7 +173,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c3", choices=["c3", "c3s", "c3t", "c1", "c2"])
-    ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf"])
+    ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -231,6 +232,9 @@ def main():
     # algorithmic bytes per launch of each kernel kind (averaged over its launches in a step)
     if args.scheme == "muscl":
         algo = {"grad_limit": ALGO_BYTES["grad_limit"], "edge_flux": ALGO_BYTES["edge_flux_muscl"],
+                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
+    elif args.scheme == "muscl_ms":
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_muscl_ms"],
                 "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
     elif args.scheme == "hllc":
         algo = {"edge_flux": ALGO_BYTES["edge_flux_hllc"], "cell_update": ALGO_BYTES["cell_update_euler"]}

@@ -43,8 +43,10 @@ typedef struct swe_ctx swe_ctx; /* opaque; owns every host and device allocation
 enum { SWE_OK = 0, SWE_ERR_ARG = -1, SWE_ERR_MESH = -2, SWE_ERR_CUDA = -3, SWE_ERR_STATE = -4,
        SWE_ERR_NOMEM = -5 };
 /* scheme: first-order HLLC + Euler (eq. 6-14); MUSCL = least-squares gradients +
- * cell limiter + HLLC + Heun RK2 (north_star); WAF + Euler (eq. 15-21). */
-enum { SWE_HLLC = 0, SWE_MUSCL = 1, SWE_WAF = 2 };
+ * cell limiter + HLLC + Heun RK2 (north_star); WAF + Euler (eq. 15-21); MUSCL_MS = the paper's own
+ * multislope MUSCL, eq. 22-25 PAPER.md:396-420 (upwind-average slopes, beta limiter: beta = 1
+ * MINBEE, 2 SUPERBEE) + HLLC + Heun RK2 (reading R17). */
+enum { SWE_HLLC = 0, SWE_MUSCL = 1, SWE_WAF = 2, SWE_MUSCL_MS = 3 };
 /* boundary kinds (fixed level: PAPER.md:518, 548, reading R11) */
 enum { SWE_BC_WALL = 0, SWE_BC_INFLOW_Q = 1, SWE_BC_LEVEL = 2, SWE_BC_TRANSMISSIVE = 3 };
 enum { SWE_RENUM_NONE = 0, SWE_RENUM_HILBERT = 1 };
@@ -88,7 +90,7 @@ int swe_set_time(swe_ctx* ctx, double t);
  * call synchronises the stream and returns the simulated time and the last dt.  With zones built
  * (swe_zones_create) the step runs zone-wise with pack/unpack of the ghost cells every stage.
  * Errors: SWE_ERR_ARG (nsteps < 0, cfl <= 0, unknown scheme), SWE_ERR_STATE (zones built with too
- * few ghost layers for the scheme: WAF needs 2), SWE_ERR_CUDA. */
+ * few ghost layers for the scheme: WAF and MUSCL_MS need 2), SWE_ERR_CUDA. */
 int swe_step(swe_ctx* ctx, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out);
 
 /* Zone decomposition resident on this GPU.

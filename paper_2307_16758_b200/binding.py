@@ -14,10 +14,10 @@ from . import build as _build
 
 SWE_OK = 0
 SWE_ERR_ARG, SWE_ERR_MESH, SWE_ERR_CUDA, SWE_ERR_STATE, SWE_ERR_NOMEM = -1, -2, -3, -4, -5
-SWE_HLLC, SWE_MUSCL, SWE_WAF = 0, 1, 2
+SWE_HLLC, SWE_MUSCL, SWE_WAF, SWE_MUSCL_MS = 0, 1, 2, 3
 SWE_BC_WALL, SWE_BC_INFLOW_Q, SWE_BC_LEVEL, SWE_BC_TRANSMISSIVE = 0, 1, 2, 3
 SWE_RENUM_NONE, SWE_RENUM_HILBERT = 0, 1
-SCHEMES = {"hllc": SWE_HLLC, "muscl": SWE_MUSCL, "waf": SWE_WAF}
+SCHEMES = {"hllc": SWE_HLLC, "muscl": SWE_MUSCL, "waf": SWE_WAF, "muscl_ms": SWE_MUSCL_MS}
 BC_KINDS = {"wall": SWE_BC_WALL, "inflow": SWE_BC_INFLOW_Q, "level": SWE_BC_LEVEL,
             "transmissive": SWE_BC_TRANSMISSIVE}
 KERNEL_KINDS = ("dt_reduce", "grad_limit", "edge_flux", "cell_update", "pack", "unpack", "dt_finalize")

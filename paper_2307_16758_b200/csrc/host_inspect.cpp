@@ -42,6 +42,8 @@ int64_t mesh_get(const MeshArrays& M, const std::string& n, void* out, int64_t c
     if (n == "erl") return copy_out(M.erl, out, cap);
     if (n == "err") return copy_out(M.err, out, cap);
     if (n == "btag") return copy_out(M.btag, out, cap);
+    if (n == "dupw") return copy_out(M.dupw, out, cap);
+    if (n == "edlr") return copy_out(M.edlr, out, cap);
     return -2;
 }
 }  // namespace

@@ -261,6 +261,27 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         }
     }
     H.min_rin = nt > 0 ? min_rin : 0.0;
+    // distances of the multislope MUSCL (eq. 22-25, reading R17): x_upw of side k = mean of the
+    // centroids of the two other edge-neighbours (the cell's own centroid where one is missing)
+    M.dupw.assign(4 * (size_t)nt, 0.0);
+    M.edlr.assign(ne, 0.0);
+    for (int64_t i = 0; i < nt; ++i)
+        for (int k = 0; k < 3; ++k) {
+            double sx = 0.0, sy = 0.0;
+            for (int j = 0; j < 3; ++j) {
+                if (j == k) continue;
+                const int32_t nbq = M.c2c[4 * i + j];
+                if (nbq >= 0) { sx += H.cx[nbq]; sy += H.cy[nbq]; }
+                else { sx += H.cx[i]; sy += H.cy[i]; }
+            }
+            const double ux = H.cx[i] - 0.5 * sx, uy = H.cy[i] - 0.5 * sy;
+            M.dupw[4 * i + k] = std::sqrt(ux * ux + uy * uy);
+        }
+    for (int64_t d = 0; d < M.ne_int; ++d) {
+        const int32_t L = M.elr[2 * d], R = M.elr[2 * d + 1];
+        const double ux = H.cx[R] - H.cx[L], uy = H.cy[R] - H.cy[L];
+        M.edlr[d] = std::sqrt(ux * ux + uy * uy);
+    }
 
     // distinct tags and their widths (sum of edge lengths, reading R10)
     for (int64_t b = 0; b < nbe; ++b) {
@@ -415,7 +436,8 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     M.ne = M.ne_int + boff[nz];
     if (M.ne > (int64_t)INT32_MAX / 2) { err = "zoned mesh too large"; return false; }
     M.elr.resize(2 * M.ne); M.en.resize(2 * M.ne); M.elen.resize(M.ne); M.edx.resize(M.ne);
-    M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne);
+    M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne); M.edlr.resize(M.ne);
+    M.dupw.assign(4 * (size_t)ncz, 0.0);
     M.btag.assign(M.ne - M.ne_int, -1);
     std::vector<int32_t> eloc(G.ne, -1);
     for (int zi = 0; zi < nz; ++zi) {
@@ -427,7 +449,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             M.elr[2 * d] = (int32_t)(o + loc[L]);
             M.elr[2 * d + 1] = R >= 0 ? (int32_t)(o + loc[R]) : -1;
             M.en[2 * d] = G.en[2 * (int64_t)e]; M.en[2 * d + 1] = G.en[2 * (int64_t)e + 1];
-            M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e];
+            M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e]; M.edlr[d] = G.edlr[e];
             M.erl[2 * d] = G.erl[2 * (int64_t)e]; M.erl[2 * d + 1] = G.erl[2 * (int64_t)e + 1];
             M.err[2 * d] = G.err[2 * (int64_t)e]; M.err[2 * d + 1] = G.err[2 * (int64_t)e + 1];
             eloc[e] = (int32_t)d;
@@ -444,6 +466,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             M.cell_user[c] = G.cell_user[g];
             Z.src_of_cell[c] = (int32_t)g;
             M.zc[c] = G.zc[g]; M.area[c] = G.area[g]; M.rin[c] = G.rin[g];
+            for (int k = 0; k < 3; ++k) M.dupw[4 * c + k] = G.dupw[4 * g + k];
             for (int k = 0; k < 3; ++k) {
                 M.w[k][2 * c] = G.w[k][2 * g]; M.w[k][2 * c + 1] = G.w[k][2 * g + 1];
                 M.r[k][2 * c] = G.r[k][2 * g]; M.r[k][2 * c + 1] = G.r[k][2 * g + 1];

@@ -23,11 +23,13 @@ struct MeshArrays {
     std::vector<double> zc, area, rin;       // cell bed, |Omega_i|, in-radius
     std::vector<double> w[3];                // 2*nc each: least-squares weights (wx,wy) of side k
     std::vector<double> r[3];                // 2*nc each: r_{i,k} = m_e - c_i
+    std::vector<double> dupw;                // 4*nc: |x_i - x_upw| for side 0,1,2 (multislope MUSCL), pad
     // per edge
     std::vector<int32_t> elr;                // 2*ne: L cell, R cell (-1 on the boundary)
     std::vector<double> en;                  // 2*ne: unit normal, outward of L
     std::vector<double> elen, edx;           // length, WAF Delta-x
     std::vector<double> erl, err;            // 2*ne each: r_{L,e}, r_{R,e}
+    std::vector<double> edlr;                // |x_R - x_L| between the centroids (0 on the boundary)
     std::vector<int32_t> btag;               // ne-ne_int: user tag of the boundary edge (-1 = none)
 };
 

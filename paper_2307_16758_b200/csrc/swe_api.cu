@@ -93,7 +93,7 @@ struct swe_ctx {
     int64_t prof_n[NKIND] = {0};
     // grid sizes (persistent grid-stride kernels: a multiple of the SM count)
     int grid_light = 148 * 8;
-    int grid_grad = 148 * 4, grid_flux[3] = {148 * 4, 148 * 2, 148 * 2}, grid_upd = 148 * 8;
+    int grid_grad = 148 * 4, grid_flux[4] = {148 * 4, 148 * 2, 148 * 2, 148 * 2}, grid_upd = 148 * 8;
 
     Store& active() { return has_zones ? z : g; }
 };
@@ -175,6 +175,10 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.upload(&erl, M.erl.data(), (size_t)M.ne, s));
     CU(st.upload(&err, M.err.data(), (size_t)M.ne, s));
     d.elr = elr; d.en = en; d.elen = elen; d.edx = edx; d.erl = erl; d.err = err;
+    double4* dupw; double* edlr;
+    CU(st.upload(&dupw, M.dupw.data(), (size_t)M.nc, s));
+    CU(st.upload(&edlr, M.edlr.data(), (size_t)M.ne, s));
+    d.dupw = dupw; d.edlr = edlr;
     CU(st.upload(&st.d_cell_user, M.cell_user.data(), (size_t)M.nc, s));
     CU(st.alloc(&st.d_bkind, (size_t)st.nbe));
     CU(st.alloc(&st.d_bval, (size_t)st.nbe));
@@ -266,7 +270,8 @@ void run_flux(swe_ctx* c, Store& st, const double4* U, int scheme) {
         const int gr = grid_for(st.ne, c->grid_flux[scheme]);
         if (scheme == K_HLLC) k_edge_flux<K_HLLC><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
         else if (scheme == K_MUSCL) k_edge_flux<K_MUSCL><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else k_edge_flux<K_WAF><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else if (scheme == K_WAF) k_edge_flux<K_WAF><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else k_edge_flux<K_MUSCL_MS><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
     });
 }
 // mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in
@@ -380,6 +385,7 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC>, 4);
     c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2);
     c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2);
+    c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS>, 2);
     c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
@@ -539,14 +545,14 @@ int swe_set_time(swe_ctx* c, double t) {
 
 int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out) {
     if (check_ctx(c)) return SWE_ERR_ARG;
-    if (nsteps < 0 || !(cfl > 0.0) || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad step arguments");
-    if (c->has_zones && scheme == K_WAF && c->Z.nlayers < 2)
-        return fail(SWE_ERR_STATE, "WAF needs zones with at least 2 ghost layers");
+    if (nsteps < 0 || !(cfl > 0.0) || scheme < 0 || scheme > 3) return fail(SWE_ERR_ARG, "bad step arguments");
+    if (c->has_zones && (scheme == K_WAF || scheme == K_MUSCL_MS) && c->Z.nlayers < 2)
+        return fail(SWE_ERR_STATE, "WAF and the multislope MUSCL need zones with at least 2 ghost layers");
     Store& st = c->active();
     for (int s = 0; s < nsteps; ++s) {
         if (!c->min_valid) run_dt_reduce(c, st, st.A);                      // a9
         launch(c, KIND_MISC, [&] { k_dt_finalize<<<1, 1, 0, c->stream>>>(c->d_S, cfl, 1); });
-        if (scheme == K_MUSCL) {                                            // Heun RK2 (A.11)
+        if (scheme == K_MUSCL || scheme == K_MUSCL_MS) {                    // Heun RK2 (A.11)
             run_stage(c, st, st.A, nullptr, st.B, scheme, 0, false);
             run_stage(c, st, st.B, st.A, st.A, scheme, 1, true);
         } else {
@@ -586,7 +592,7 @@ int swe_step_timed(swe_ctx* c, int nsteps, double cfl, int scheme, float* ms_out
 
 int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out) {
     if (check_ctx(c)) return SWE_ERR_ARG;
-    if (which < 0 || which > 6 || scheme < 0 || scheme > 2 || reps < 1) return fail(SWE_ERR_ARG, "bad kernel selector");
+    if (which < 0 || which > 6 || scheme < 0 || scheme > 3 || reps < 1) return fail(SWE_ERR_ARG, "bad kernel selector");
     Store& st = c->active();
     const bool prof = c->profile; c->profile = false;
     // make the inputs of the timed kernel valid
@@ -672,7 +678,7 @@ int swe_gradients(swe_ctx* c, double* out) {
 
 int swe_side_fluxes(swe_ctx* c, double dt, int scheme, double* out) {
     if (check_ctx(c)) return SWE_ERR_ARG;
-    if (!out || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad arguments");
+    if (!out || scheme < 0 || scheme > 3) return fail(SWE_ERR_ARG, "bad arguments");
     if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
     double* d; int rc = out_to_user(c, out, 9 * (size_t)c->g.nc, &d); if (rc) return rc;
     k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);
@@ -685,7 +691,7 @@ int swe_side_fluxes(swe_ctx* c, double dt, int scheme, double* out) {
 
 int swe_euler_stage(swe_ctx* c, double dt, int scheme, double* h1, double* hu1, double* hv1) {
     if (check_ctx(c)) return SWE_ERR_ARG;
-    if (!h1 || !hu1 || !hv1 || scheme < 0 || scheme > 2) return fail(SWE_ERR_ARG, "bad arguments");
+    if (!h1 || !hu1 || !hv1 || scheme < 0 || scheme > 3) return fail(SWE_ERR_ARG, "bad arguments");
     if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
     const int64_t nt = c->g.nc;
     k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);

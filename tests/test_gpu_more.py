@@ -44,7 +44,7 @@ def test_limiter_parameter(beta):
 
 @pytest.mark.parametrize("kinds", [("transmissive", "transmissive"), ("inflow", "transmissive"),
                                    ("level", "level"), ("wall", "level")])
-@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45)])
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
 def test_boundary_kinds(kinds, scheme, cfl):
     """Every boundary kind (PAPER.md:286 + fixed level) on both tagged boundaries of the river case."""
     cfg = _river()
@@ -58,6 +58,24 @@ def test_boundary_kinds(kinds, scheme, cfl):
             o.step(1, cfl, scheme)
             sw.swe_step(c, 1, cfl, scheme)
             assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="%s %s step %d" % (kinds, scheme, s))
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
+@pytest.mark.parametrize("beta", [2.0, 1.0])
+def test_multislope_muscl_limiter_parameter(beta):
+    """The paper's MUSCL (eq. 22-25) with SUPERBEE (beta = 2, the paper's choice) and MINBEE."""
+    cfg = config0()
+    cfg["params"] = dict(cfg["params"], beta=beta)
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        for s in range(60):
+            sw.swe_set_state(c, *o.get_state())
+            o.step(1, 0.45, "muscl_ms")
+            sw.swe_step(c, 1, 0.45, "muscl_ms")
+            assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="ms beta %g step %d" % (beta, s))
     finally:
         sw.swe_mesh_destroy(c)
         o.close()

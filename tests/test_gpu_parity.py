@@ -61,7 +61,7 @@ def test_single_passes_match_oracle(name):
         c2c, c2e = o.cell_topology()
         eg = o.edge_geometry()
         edges = np.unique(np.linspace(0, o.ne - 1, 1200).astype(np.int64))
-        for scheme in ("hllc", "muscl", "waf"):
+        for scheme in ("hllc", "muscl", "waf", "muscl_ms"):
             fg = sw.swe_side_fluxes(c, dt, scheme)
             got, ref = [], []
             for e in edges:
@@ -83,7 +83,7 @@ def test_single_passes_match_oracle(name):
 
 
 @pytest.mark.parametrize("name", ["c0", "ritter", "wave", "c1", "lake", "river"])
-@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45)])
+@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45), ("muscl_ms", 0.45)])
 def test_per_step_and_run_parity_small(name, scheme, cfl):
     """Per step: both sides start every step from the oracle's state (<= 1e-11).  Then a free run
     of the same length from the initial state (<= 1e-8)."""
@@ -119,7 +119,7 @@ def test_renumbering_is_invisible():
     a = sw.create_from_config(cfg, sw.SWE_RENUM_NONE)
     b = sw.create_from_config(cfg, sw.SWE_RENUM_HILBERT)
     try:
-        for scheme, cfl in (("muscl", 0.45), ("waf", 0.45), ("hllc", 0.9)):
+        for scheme, cfl in (("muscl", 0.45), ("waf", 0.45), ("hllc", 0.9), ("muscl_ms", 0.45)):
             ta = sw.swe_step(a, 25, cfl, scheme)
             tb = sw.swe_step(b, 25, cfl, scheme)
             assert ta == tb
@@ -208,7 +208,7 @@ def test_config3_reduced_long_run():
     """configs[3] structure at reduced size (same generator: banded river mesh, inflow Q, fixed
     level, partly dry, Manning by zone), 200 steps MUSCL and HLLC; inflow volume balance."""
     cfg = config3(length=6400.0, half_width=1000.0, w2=40.0, n4=6, n8=4)
-    for scheme, cfl in (("muscl", 0.45), ("hllc", 0.9)):
+    for scheme, cfl in (("muscl", 0.45), ("hllc", 0.9), ("muscl_ms", 0.45)):
         o, c = _pair(cfg)
         try:
             o.step(1, cfl, scheme)

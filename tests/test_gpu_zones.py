@@ -18,14 +18,14 @@ def _river():
 
 
 @pytest.mark.parametrize("nz,nl", [(4, 1), (8, 2), (32, 2), (4, 3)])
-@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45)])
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
 def test_zoned_run_is_bit_identical(nz, nl, scheme, cfl):
     cfg = _river()
     a = sw.create_from_config(cfg)
     b = sw.create_from_config(cfg)
     try:
         sw.swe_zones_create(b, nz, nl)
-        if scheme == "waf" and nl < 2:
+        if scheme in ("waf", "muscl_ms") and nl < 2:
             with pytest.raises(sw.SweError) as e:
                 sw.swe_step(b, 1, cfl, scheme)
             assert e.value.code == sw.SWE_ERR_STATE
