@@ -163,3 +163,33 @@ def test_time_accumulates_and_can_be_set():
     finally:
         sw.swe_mesh_destroy(c)
         o.close()
+
+
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_dry_cells_with_leftover_momentum(scheme, cfl):
+    """Cells without water are skipped by the gradient and flux kernels (their records are exactly
+    zero by A.3.5 / A.5-A.9).  A user state may still carry momentum in such cells, and depths
+    between 0 and h_dry are NOT skipped: both must behave as in the oracle."""
+    cfg = lake_case(n=40)
+    rng = np.random.default_rng(5)
+    h = cfg["h"].copy()
+    dry = h == 0.0
+    assert dry.sum() > 100
+    hu = np.where(dry, rng.normal(size=h.size), 0.0)          # leftover momentum in dry cells
+    hv = np.where(dry, rng.normal(size=h.size), 0.0)
+    thin = rng.random(h.size) < 0.3
+    h = np.where(dry & thin, 5e-7, h)                          # below h_dry but not zero
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        o.set_state(h, hu, hv)
+        for s in range(10):
+            sw.swe_set_state(c, *o.get_state())
+            o.step(1, cfl, scheme)
+            sw.swe_step(c, 1, cfl, scheme)
+            assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="dry %s step %d" % (scheme, s))
+        go, gg = o.gradients(), sw.swe_gradients(c)
+        assert np.abs(gg - go).max() <= 1e-11 * max(np.abs(go).max(), 1e-3)
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
