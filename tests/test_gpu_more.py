@@ -193,3 +193,58 @@ def test_dry_cells_with_leftover_momentum(scheme, cfl):
     finally:
         sw.swe_mesh_destroy(c)
         o.close()
+
+
+def test_error_paths_leave_the_context_usable():
+    cfg = lake_case(n=20)
+    c = sw.create_from_config(cfg)
+    try:
+        ref = sw.swe_get_state(c)
+        for call, code in [
+            (lambda: sw.swe_set_bc(c, -1, "wall", 0.0), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_set_bc(c, 1, 9, 0.0), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_set_params(c, -9.81, 1e-6, 1e-3, 1.0), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_zones_create(c, 3, 2), sw.SWE_ERR_ARG),          # RCB needs a power of two
+            (lambda: sw.swe_zones_create(c, 4, 0), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_zones_create(c, 2, 2, np.full(cfg["h"].size, 5, np.int32)), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_pack_ghosts(c, -1), sw.SWE_ERR_STATE),           # no zones yet
+            (lambda: sw.swe_zone_stats(c), sw.SWE_ERR_STATE),
+            (lambda: sw.swe_kernel_timed(c, 99, "muscl", 1), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_step(c, -1, 0.5, "hllc"), sw.SWE_ERR_ARG),
+            (lambda: sw.swe_compute_dt(c, 0.0), sw.SWE_ERR_ARG),
+        ]:
+            with pytest.raises(sw.SweError) as e:
+                call()
+            assert e.value.code == code and str(e.value)
+        for x, y in zip(ref, sw.swe_get_state(c)):
+            assert np.array_equal(x, y)
+        # explicit zone map (not RCB), then single-pass calls are refused while zones exist
+        zmap = (np.arange(cfg["h"].size) % 3).astype(np.int32)
+        sw.swe_zones_create(c, 3, 2, zmap)
+        with pytest.raises(sw.SweError) as e:
+            sw.swe_gradients(c)
+        assert e.value.code == sw.SWE_ERR_STATE
+        with pytest.raises(sw.SweError):
+            sw.swe_pack_ghosts(c, 7)
+        a = sw.create_from_config(cfg)
+        sw.swe_step(a, 15, 0.45, "muscl")
+        sw.swe_step(c, 15, 0.45, "muscl")                   # scattered zones: still bit-identical
+        for x, y in zip(sw.swe_get_state(a), sw.swe_get_state(c)):
+            assert np.array_equal(x, y)
+        sw.swe_mesh_destroy(a)
+    finally:
+        sw.swe_mesh_destroy(c)
+
+
+def test_mesh_errors_through_the_gpu_entry_point():
+    x = np.array([0.0, 1.0, 0.0, 1.0]); y = np.array([0.0, 0.0, 1.0, 1.0]); z = np.zeros(4)
+    with pytest.raises(sw.SweError) as e:
+        sw.swe_mesh_create(x, y, z, np.array([[0, 1, 9]], np.int32))
+    assert e.value.code == sw.SWE_ERR_MESH
+    with pytest.raises(sw.SweError) as e:
+        sw.swe_mesh_create(x, y, z, np.array([[0, 1, 2], [1, 3, 2]], np.int32),
+                           np.array([[1, 2]], np.int32), np.array([1], np.int32))
+    assert e.value.code == sw.SWE_ERR_MESH and "boundary" in str(e.value)
+    with pytest.raises(sw.SweError) as e:
+        sw.swe_mesh_create(x, y, z, np.array([[0, 1, 2]], np.int32), renumber=5)
+    assert e.value.code == sw.SWE_ERR_ARG
