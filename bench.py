@@ -5,12 +5,14 @@ kernel, an end-to-end figure through the C ABI with host buffers, and the CPU or
 it.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload c3|c3s|c1|c2]
-                    [--scheme muscl|hllc|waf] [--zones Z --layers L]
+                    [--scheme muscl|hllc|waf|muscl_ms] [--zones Z --layers L] [--transport p2p|staged]
 
 One "step" = one full time step (CFL min-reduction, both Heun stages: gradient+limiter, edge flux,
-cell update) over every cell of the mesh.  N > 1 (torchrun): one independent replica of the
-workload per GPU ("replicas only": the multi-GPU halo exchange is row f3 of the scope table, not
-built), weak scaling, value = all ranks' cell-updates / max-over-ranks time.
+cell update) over every cell of the mesh.  N > 1 (torchrun): the SAME mesh split into zones over
+the N ranks (strong scaling; paper_2307_16758_b200/dist.py): per stage one halo exchange of the
+ghost cells (one kernel storing into the peers' ghost ranges over NVLink peer memory, or pack ->
+NCCL all-to-all -> unpack with --transport staged) and per step one all-reduce(min) of dt;
+value = cells x steps / max-over-ranks device time.  --replicas runs N independent copies instead.
 Prints ONE JSON line on rank 0.
 """
 import argparse
@@ -166,6 +168,125 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workload):
+    """Per-kernel figures from the CUDA-event profile of the timed step loop (swe_get_profile)."""
+    kern = {}
+    tot_ms = sum(v[0] for v in prof.values())
+    for k, (kms, n) in prof.items():
+        if n:
+            kern[k] = {"ms_per_launch": kms / n, "launches_per_step": n / steps, "share": kms / tot_ms}
+    # algorithmic bytes per launch of each kernel kind (averaged over its launches in a step)
+    if scheme == "muscl":
+        algo = {"grad_limit": ALGO_BYTES["grad_limit"], "edge_flux": ALGO_BYTES["edge_flux_muscl"],
+                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
+    elif scheme == "muscl_ms":
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_muscl_ms"],
+                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
+    elif scheme == "hllc":
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_hllc"], "cell_update": ALGO_BYTES["cell_update_euler"]}
+    else:
+        algo = {"edge_flux": ALGO_BYTES["edge_flux_waf"], "cell_update": ALGO_BYTES["cell_update_euler"]}
+    for k in algo:
+        if k in kern:
+            kern[k]["algo_GBps"] = algo[k] * cells / (kern[k]["ms_per_launch"] * 1e-3) / 1e9
+            kern[k]["frac_of_peak"] = kern[k]["algo_GBps"] / peak
+    dom = max((k for k in algo if k in kern), key=lambda k: kern[k]["share"])
+    tt = traffic_table()
+    traffic = tt.get((workload, dom + "_" + scheme), tt.get((workload, dom)))
+    step_bytes = ALGO_BYTES["step_" + scheme]
+    rate = cells / (step_ms * 1e-3)
+    return {
+        "bound": "hbm", "kernel": dom, "achieved": kern[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
+        "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+        "algo_bytes_per_launch": algo[dom] * cells,
+        "step_algo_GBps": step_bytes * rate / 1e9,
+        "step_frac_of_peak": step_bytes * rate / 1e9 / peak,
+        "step_frac_of_8TBps": step_bytes * rate / 1e9 / 8000.0,
+        "kernels": kern,
+    }
+
+
+def run_dist(args, rank, world, local, cfg, desc, cfl):
+    """N > 1: the mesh split into zones over the ranks (strong scaling), one halo exchange per stage
+    over NVLink peer memory (or pack -> NCCL all-to-all -> unpack) and one all-reduce(min) for dt."""
+    import torch
+    from paper_2307_16758_b200 import dist as swdist
+    import paper_2307_16758_b200 as sw
+
+    S = swdist.DistSolver(cfg, nzones=args.zones if args.zones > 0 else None, nlayers=args.layers,
+                          transport=args.transport)
+    nt = S.ncell
+    info = sw.swe_mesh_info(S.ctx)
+    owned = sum(sw.swe_zone_describe_counts(S.ctx, z)[0] for z in range(*swdist.shard_units(S.nzones, rank, world)))
+    S.step(args.warmup, cfl, args.scheme)
+    torch.cuda.synchronize()
+    swdist.barrier()
+    l0 = sw.swe_get_stats(S.ctx)
+    clk = ClockSampler(local)
+    clk.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    S.step(args.steps, cfl, args.scheme)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    l1 = sw.swe_get_stats(S.ctx)
+    swdist.barrier()
+    ms_max = swdist.reduce_max(ms)
+    value = nt * args.steps / (ms_max * 1e-3)
+    launches = swdist.reduce_sum(float(l1["kernel_launches"] - l0["kernel_launches"]))
+    halo = swdist.reduce_sum(float(l1["halo_bytes"] - l0["halo_bytes"])) / args.steps
+
+    # per-kernel CUDA events on this rank's launches (rank 0 reports its own share of the mesh)
+    sw.swe_set_profile(S.ctx, True)
+    S.step(args.steps, cfl, args.scheme)
+    prof = sw.swe_get_profile(S.ctx)
+    sw.swe_set_profile(S.ctx, False)
+    clocks = clk.stop()
+    peak, peak_src = hbm_peak()
+    roofline = kernel_roofline(prof, args.steps, args.scheme, owned, ms / args.steps, peak, peak_src, args.workload)
+    roofline["note"] = "rank 0's kernels over the %d cells its zones own (ghost cells not counted)" % owned
+
+    # end to end with HOST buffers: every rank uploads the full state, steps, reads its own cells back
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    hbuf = [torch.zeros(nt, dtype=torch.float64).pin_memory() for _ in range(3)]
+    full = S.get_state()
+    for b, f in zip(hbuf, full):
+        b.copy_(torch.from_numpy(f))
+    for _ in range(2):
+        S.set_state(*hbuf); S.step(1, cfl, args.scheme); S.get_state_local(*hbuf)
+    torch.cuda.synchronize()
+    swdist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        S.set_state(*hbuf)
+        S.step(1, cfl, args.scheme)
+        S.get_state_local(*hbuf)
+    torch.cuda.synchronize()
+    e2e_s = swdist.reduce_max(time.perf_counter() - t0)
+    e2e = {"value": nt * e2e_steps / e2e_s, "unit": "cell-updates/s", "steps": e2e_steps,
+           "h2d_bytes_per_step": 3 * 8 * nt * world, "d2h_bytes_per_step": 3 * 8 * nt * world,
+           "what": "per step and rank: swe_set_state(full state, pinned host) + one distributed step + "
+                   "swe_get_state(pinned host; the rank's own cells are filled)"}
+    S.close()
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "cell-updates/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "cells": nt, "edges": info["nedge"], "scheme": args.scheme, "cfl": cfl,
+                       "l2": "inputs larger than L2 per rank" if nt / world > 2_000_000 else
+                             "a rank's share may fit L2 at this size",
+                       "parallelism": "zones over %d ranks (%d zones, %d ghost layers), halo transport %s, "
+                                      "all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport),
+                       "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo},
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": None,
+            "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line))
+    swdist.finalize()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -176,6 +297,8 @@ def main():
     ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--transport", default="p2p", choices=["p2p", "staged"])
+    ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
     args = ap.parse_args()
@@ -196,6 +319,8 @@ def main():
 
     cfg, desc = build_workload(args.workload)
     cfl = 0.9 if args.scheme == "hllc" else 0.45
+    if world > 1 and not args.replicas:
+        return run_dist(args, rank, world, local, cfg, desc, cfl)
     ctx = sw.create_from_config(cfg)
     info = sw.swe_mesh_info(ctx)
     nt = info["ncell"]
@@ -224,39 +349,7 @@ def main():
     sw.swe_set_profile(ctx, False)
     clocks = clk.stop()
     peak, peak_src = hbm_peak()
-    kern = {}
-    tot_ms = sum(v[0] for v in prof.values())
-    for k, (kms, n) in prof.items():
-        if n:
-            kern[k] = {"ms_per_launch": kms / n, "launches_per_step": n / args.steps, "share": kms / tot_ms}
-    # algorithmic bytes per launch of each kernel kind (averaged over its launches in a step)
-    if args.scheme == "muscl":
-        algo = {"grad_limit": ALGO_BYTES["grad_limit"], "edge_flux": ALGO_BYTES["edge_flux_muscl"],
-                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
-    elif args.scheme == "muscl_ms":
-        algo = {"edge_flux": ALGO_BYTES["edge_flux_muscl_ms"],
-                "cell_update": 0.5 * (ALGO_BYTES["cell_update_stage"] + ALGO_BYTES["cell_update_final"])}
-    elif args.scheme == "hllc":
-        algo = {"edge_flux": ALGO_BYTES["edge_flux_hllc"], "cell_update": ALGO_BYTES["cell_update_euler"]}
-    else:
-        algo = {"edge_flux": ALGO_BYTES["edge_flux_waf"], "cell_update": ALGO_BYTES["cell_update_euler"]}
-    for k in algo:
-        if k in kern:
-            kern[k]["algo_GBps"] = algo[k] * nt / (kern[k]["ms_per_launch"] * 1e-3) / 1e9
-            kern[k]["frac_of_peak"] = kern[k]["algo_GBps"] / peak
-    dom = max((k for k in algo if k in kern), key=lambda k: kern[k]["share"])
-    tt = traffic_table()
-    traffic = tt.get((args.workload, dom + "_" + args.scheme), tt.get((args.workload, dom)))
-    step_bytes = ALGO_BYTES["step_" + args.scheme]
-    roofline = {
-        "bound": "hbm", "kernel": dom, "achieved": kern[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
-        "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
-        "algo_bytes_per_launch": algo[dom] * nt,
-        "step_algo_GBps": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9,
-        "step_frac_of_peak": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9 / peak,
-        "step_frac_of_8TBps": step_bytes * (nt * args.steps / (ms * 1e-3)) / 1e9 / 8000.0,
-        "kernels": kern,
-    }
+    roofline = kernel_roofline(prof, args.steps, args.scheme, nt, ms / args.steps, peak, peak_src, args.workload)
 
     # ---- end to end through the C ABI with HOST buffers: every step copies the state host->device
     # (pinned memory), advances one step and reads the state back ----

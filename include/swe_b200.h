@@ -79,8 +79,8 @@ int swe_set_manning(swe_ctx* ctx, const double* n_cell);
  * spread uniformly over the tag's total width] for SWE_BC_INFLOW_Q, free-surface level [m] for
  * SWE_BC_LEVEL; ignored otherwise. */
 int swe_set_bc(swe_ctx* ctx, int tag, int kind, double value);
-/* state, nt values each, user order.  SWE_ERR_STATE if any h is NaN or negative.  Resets t to 0
- * only if reset_time != 0 in swe_set_time; swe_set_state itself leaves t unchanged. */
+/* state, nt values each, user order.  SWE_ERR_STATE if any h is NaN or negative (the state is then
+ * left as it was).  The simulated time t is not touched; use swe_set_time. */
 int swe_set_state(swe_ctx* ctx, const double* h, const double* hu, const double* hv);
 int swe_get_state(const swe_ctx* ctx, double* h, double* hu, double* hv);
 int swe_set_time(swe_ctx* ctx, double t);
@@ -114,6 +114,67 @@ int swe_zone_describe(const swe_ctx* ctx, int zone, int64_t* nowned, int64_t* ng
 int swe_zone_cells(const swe_ctx* ctx, int zone, int32_t* cells, int32_t* layer);
 int swe_zone_links(const swe_ctx* ctx, int zone, int32_t* src, int32_t* start, int32_t* count);
 int swe_zone_sendlist(const swe_ctx* ctx, int zone, int link, int32_t* send_idx);
+
+/* ---- zones distributed over ranks: one process per GPU (scope row f3) -------
+ * The paper runs one MPI rank + one GPU per sub-domain and exchanges the ghost cells of U every
+ * step.  Here rank r of nranks holds the zones [zone_begin[r], zone_begin[r+1])
+ * of the SAME decomposition every rank builds from the same mesh (so no set-up message is needed:
+ * each rank derives its own lists and its peers' independently, in the same order).  The library
+ * never calls a communication library: the caller (paper_2307_16758_b200/dist.py, over
+ * torch.distributed) moves or synchronises, the library packs, pushes and unpacks.  Per step:
+ *     exchange(buffer 0); swe_dist_local_min -> all-reduce(min) -> swe_dist_begin_step;
+ *     swe_dist_stage(scheme, 0); [Heun schemes: exchange(buffer 1); barrier; swe_dist_stage(scheme, 1)]
+ * with exchange = swe_halo_push (peer memory, one kernel) or swe_halo_pack -> transfer ->
+ * swe_halo_unpack.  swe_step refuses (SWE_ERR_STATE) while the zones are distributed.
+ * swe_set_state / swe_set_manning / swe_set_bc are called on every rank with the same full-mesh
+ * arguments; swe_get_state writes only the cells owned by this rank's zones and leaves the other
+ * entries of the output arrays untouched.  nlayers >= 2 is required for MUSCL, WAF and MUSCL_MS
+ * (no gradient exchange between ranks); nlayers = 1 serves HLLC.
+ *   zone_begin : nranks+1 non-decreasing zone ids from 0 to nzones (host pointer); may be NULL when
+ *                nranks == 1.  Errors: SWE_ERR_ARG. */
+int swe_zones_create_dist(swe_ctx* ctx, int nzones, int nlayers, const int32_t* zone_of_cell,
+                          int nranks, int rank, const int32_t* zone_begin);
+/* cells this rank sends to / receives from each peer per exchange (nranks entries each, host
+ * pointers, either may be NULL); the halo buffers below hold 3 doubles (h, hu, hv) per cell, the
+ * block of peer p starting at 3 * (sum of the counts of the peers before it). */
+int swe_halo_counts(const swe_ctx* ctx, int64_t* send_cells, int64_t* recv_cells);
+/* a10 across ranks: gather the send cells of state buffer `buffer` (0 = U / stage-1 input,
+ * 1 = the Heun stage buffer U') into sendbuf (device pointer, 3 * total send cells doubles),
+ * ordered by peer, then by (destination zone, source zone), then by position in the link. */
+int swe_halo_pack(swe_ctx* ctx, int buffer, double* sendbuf);
+/* copy recvbuf (device pointer, same ordering seen from the receiving side) into the contiguous
+ * ghost ranges of `buffer`, then refresh the ghosts fed by zones resident on this rank. */
+int swe_halo_unpack(swe_ctx* ctx, int buffer, const double* recvbuf);
+/* Exchange over peer memory (NVLink / NVSwitch peer stores; PAPER.md:460's send buffer + in-place
+ * receive fused into ONE kernel): swe_peer_export returns the CUDA IPC handles of this rank's two
+ * state buffers (128 bytes: buffer 0 then buffer 1); the caller all-gathers them and calls
+ * swe_peer_import(peer, handles of that peer) on every rank for every other rank.  Peers that live
+ * in the same process (tests) are connected with swe_peer_raw / swe_peer_set_raw instead.
+ * swe_halo_push(buffer) then stores every send cell's record straight into the ghost range of the
+ * rank that needs it and refreshes the ghosts fed by resident zones.  It is asynchronous on the
+ * context's stream and does NOT synchronise the ranks: before a rank reads its ghosts, every peer's
+ * push must have completed, and before a push, the target must have finished reading the ghosts of
+ * that buffer -- the caller orders this with a stream-ordered collective (the all-reduce of dt after
+ * the push of buffer 0, a barrier after the push of buffer 1; dist.py).  Errors: SWE_ERR_STATE (no
+ * zones / a peer with a non-empty send list not imported), SWE_ERR_CUDA (IPC failure). */
+int swe_peer_export(swe_ctx* ctx, unsigned char* handles /* 128 bytes, host */);
+int swe_peer_import(swe_ctx* ctx, int peer, const unsigned char* handles /* 128 bytes, host */);
+int swe_peer_raw(swe_ctx* ctx, void** buf0, void** buf1);
+int swe_peer_set_raw(swe_ctx* ctx, int peer, void* buf0, void* buf1);
+int swe_halo_push(swe_ctx* ctx, int buffer);
+/* a9 across ranks: min over this rank's owned wet cells of R_i / lambda_i (eq. 5), +inf if none,
+ * written to min_out (DEVICE pointer, 1 double; no host synchronisation).  After the last stage of
+ * a step the value is already there (folded into the update). */
+int swe_dist_local_min(swe_ctx* ctx, double* min_out);
+/* dt = cfl * (*min_in) (DEVICE pointer: the all-reduced minimum; +inf -> dt = 0, the step is a
+ * no-op), t += dt. */
+int swe_dist_begin_step(swe_ctx* ctx, const double* min_in, double cfl);
+/* one stage of the scheme on this rank's zones: stage 0 reads buffer 0 (Heun: writes buffer 1;
+ * Euler schemes: updates buffer 0 in place and end the step); stage 1 (Heun only) reads buffer 1
+ * and writes U^{n+1} = (U^n + E(U'))/2 to buffer 0.  The ghosts of the buffer read must be current. */
+int swe_dist_stage(swe_ctx* ctx, int scheme, int stage);
+/* simulated time and last dt (host pointers; synchronises the stream). */
+int swe_get_time(swe_ctx* ctx, double* t_out, double* last_dt_out);
 
 /* ---- single passes of the hot path, exposed for parity tests and kernel timing -------------
  * (SURVEY.md section 8(a) rows a2, a3-a7, a8, a9).  They act on the current state, un-zoned. */
@@ -158,6 +219,10 @@ int swe_host_mesh_build(void** out, int64_t nv, const double* x, const double* y
                         int64_t nt, const int32_t* tri, int64_t nb, const int32_t* bedge,
                         const int32_t* btag, int renumber);
 int swe_host_zones_build(void* handle, int nzones, int nlayers, const int32_t* zone_of_cell);
+/* the distributed variant (swe_zones_create_dist's host half): adds the names "zone_rank",
+ * "rsend_idx", "rsend_dst", "rsend_peer", "rrecv_idx", "rsend_off", "rrecv_off" to swe_host_get. */
+int swe_host_zones_build_dist(void* handle, int nzones, int nlayers, const int32_t* zone_of_cell,
+                              int nranks, int rank, const int32_t* zone_begin);
 void swe_host_mesh_free(void* handle);
 int64_t swe_host_get(void* handle, const char* name, void* out, int64_t capacity_bytes);
 const char* swe_host_last_error(void);

@@ -45,6 +45,19 @@ SIGNATURES = {
     "swe_zone_cells": (C.c_int, [_vp, C.c_int, _vp, _vp]),
     "swe_zone_links": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
     "swe_zone_sendlist": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
+    "swe_zones_create_dist": (C.c_int, [_vp, C.c_int, C.c_int, _vp, C.c_int, C.c_int, _vp]),
+    "swe_halo_counts": (C.c_int, [_vp, _vp, _vp]),
+    "swe_halo_pack": (C.c_int, [_vp, C.c_int, _vp]),
+    "swe_halo_unpack": (C.c_int, [_vp, C.c_int, _vp]),
+    "swe_peer_export": (C.c_int, [_vp, _vp]),
+    "swe_peer_import": (C.c_int, [_vp, C.c_int, _vp]),
+    "swe_peer_raw": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "swe_peer_set_raw": (C.c_int, [_vp, C.c_int, _vp, _vp]),
+    "swe_halo_push": (C.c_int, [_vp, C.c_int]),
+    "swe_dist_local_min": (C.c_int, [_vp, _vp]),
+    "swe_dist_begin_step": (C.c_int, [_vp, _vp, C.c_double]),
+    "swe_dist_stage": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "swe_get_time": (C.c_int, [_vp, _dp, _dp]),
     "swe_compute_dt": (C.c_int, [_vp, C.c_double, _dp]),
     "swe_gradients": (C.c_int, [_vp, _vp]),
     "swe_side_fluxes": (C.c_int, [_vp, C.c_double, C.c_int, _vp]),
@@ -57,6 +70,7 @@ SIGNATURES = {
     "swe_last_error": (C.c_char_p, []),
     "swe_host_mesh_build": (C.c_int, [C.POINTER(_vp), C.c_int64, _vp, _vp, _vp, C.c_int64, _vp, C.c_int64, _vp, _vp, C.c_int]),
     "swe_host_zones_build": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
+    "swe_host_zones_build_dist": (C.c_int, [_vp, C.c_int, C.c_int, _vp, C.c_int, C.c_int, _vp]),
     "swe_host_mesh_free": (None, [_vp]),
     "swe_host_get": (C.c_int64, [_vp, C.c_char_p, _vp, C.c_int64]),
     "swe_host_last_error": (C.c_char_p, []),
@@ -202,6 +216,13 @@ def swe_zone_stats(ctx):
     return {"send_cells_total": a.value, "bytes_per_exchange": b.value, "ghost_cells_total": c.value}
 
 
+def swe_zone_describe_counts(ctx, zone):
+    """(owned cells, ghost cells, links) of one zone."""
+    no, ng, nl = C.c_int64(), C.c_int64(), C.c_int64()
+    _check(lib().swe_zone_describe(ctx, int(zone), C.byref(no), C.byref(ng), C.byref(nl)))
+    return no.value, ng.value, nl.value
+
+
 def swe_zone_describe(ctx, zone):
     """counts + arrays of one zone (swe_zone_describe / _cells / _links / _sendlist)."""
     no, ng, nl = C.c_int64(), C.c_int64(), C.c_int64()
@@ -219,6 +240,71 @@ def swe_zone_describe(ctx, zone):
         _check(lib().swe_zone_sendlist(ctx, int(zone), j, _ptr(sl)))
         links.append((int(src[j]), int(start[j]), int(cnt[j]), sl))
     return {"nowned": no.value, "cells": cells, "layer": layer, "links": links}
+
+
+# ---- zones distributed over ranks (the caller moves / synchronises; see dist.py) ----
+def swe_zones_create_dist(ctx, nzones, nlayers, zone_of_cell, nranks, rank, zone_begin):
+    z = _i32(zone_of_cell)
+    zb = None if zone_begin is None else np.ascontiguousarray(zone_begin, dtype=np.int32)
+    _check(lib().swe_zones_create_dist(ctx, int(nzones), int(nlayers), _ptr(z), int(nranks), int(rank), _ptr(zb)))
+
+
+def swe_halo_counts(ctx, nranks):
+    s, r = np.zeros(nranks, np.int64), np.zeros(nranks, np.int64)
+    _check(lib().swe_halo_counts(ctx, _ptr(s), _ptr(r)))
+    return s, r
+
+
+def swe_halo_pack(ctx, buffer, sendbuf):
+    _check(lib().swe_halo_pack(ctx, int(buffer), _ptr(sendbuf)))
+
+
+def swe_halo_unpack(ctx, buffer, recvbuf):
+    _check(lib().swe_halo_unpack(ctx, int(buffer), _ptr(recvbuf)))
+
+
+def swe_peer_export(ctx):
+    h = np.zeros(128, np.uint8)
+    _check(lib().swe_peer_export(ctx, _ptr(h)))
+    return h
+
+
+def swe_peer_import(ctx, peer, handles):
+    h = np.ascontiguousarray(handles, dtype=np.uint8)
+    assert h.size == 128
+    _check(lib().swe_peer_import(ctx, int(peer), _ptr(h)))
+
+
+def swe_peer_raw(ctx):
+    a, b = _vp(), _vp()
+    _check(lib().swe_peer_raw(ctx, C.byref(a), C.byref(b)))
+    return a.value, b.value
+
+
+def swe_peer_set_raw(ctx, peer, buf0, buf1):
+    _check(lib().swe_peer_set_raw(ctx, int(peer), buf0, buf1))
+
+
+def swe_halo_push(ctx, buffer):
+    _check(lib().swe_halo_push(ctx, int(buffer)))
+
+
+def swe_dist_local_min(ctx, min_out):
+    _check(lib().swe_dist_local_min(ctx, _ptr(min_out)))
+
+
+def swe_dist_begin_step(ctx, min_in, cfl):
+    _check(lib().swe_dist_begin_step(ctx, _ptr(min_in), float(cfl)))
+
+
+def swe_dist_stage(ctx, scheme, stage):
+    _check(lib().swe_dist_stage(ctx, _scheme(scheme), int(stage)))
+
+
+def swe_get_time(ctx):
+    t, dt = C.c_double(), C.c_double()
+    _check(lib().swe_get_time(ctx, C.byref(t), C.byref(dt)))
+    return t.value, dt.value
 
 
 def swe_compute_dt(ctx, cfl):
@@ -299,6 +385,8 @@ def create_from_config(cfg, renumber=SWE_RENUM_HILBERT, cuda_stream=None):
 _HOST_DTYPES = {"cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": np.int32, "btag": np.int32,
                 "user_cell": np.int32, "zone_of": np.int32, "send_idx": np.int32, "recv_idx": np.int32,
                 "src_of_cell": np.int32, "link_src": np.int32, "link_dst": np.int32, "tags": np.int32,
+                "zone_rank": np.int32, "rsend_idx": np.int32, "rsend_dst": np.int32, "rsend_peer": np.int32,
+                "rrecv_idx": np.int32, "rsend_off": np.int64, "rrecv_off": np.int64,
                 "link_off": np.int64, "zone_offset": np.int64, "zone_nowned": np.int64, "zone_ncells": np.int64}
 
 
@@ -318,6 +406,14 @@ def swe_host_mesh_build(x, y, zb, tri, bedge=None, btag=None, renumber=SWE_RENUM
 def swe_host_zones_build(handle, nzones, nlayers, zone_of_cell=None):
     z = _i32(zone_of_cell)
     rc = lib().swe_host_zones_build(handle, int(nzones), int(nlayers), _ptr(z))
+    if rc != SWE_OK:
+        raise SweError(rc, lib().swe_host_last_error().decode())
+
+
+def swe_host_zones_build_dist(handle, nzones, nlayers, zone_of_cell, nranks, rank, zone_begin):
+    z = _i32(zone_of_cell)
+    zb = None if zone_begin is None else np.ascontiguousarray(zone_begin, dtype=np.int32)
+    rc = lib().swe_host_zones_build_dist(handle, int(nzones), int(nlayers), _ptr(z), int(nranks), int(rank), _ptr(zb))
     if rc != SWE_OK:
         raise SweError(rc, lib().swe_host_last_error().decode())
 

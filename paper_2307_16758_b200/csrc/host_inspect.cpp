@@ -74,6 +74,16 @@ int swe_host_zones_build(void* hh, int nzones, int nlayers, const int32_t* zone_
     h->zones = true;
     return SWE_OK;
 }
+int swe_host_zones_build_dist(void* hh, int nzones, int nlayers, const int32_t* zone_of_cell, int nranks,
+                              int rank, const int32_t* zone_begin) {
+    HostHandle* h = (HostHandle*)hh;
+    if (!h) { h_err = "null handle"; return SWE_ERR_ARG; }
+    std::string err;
+    h->zones = false;
+    if (!build_zones(h->H, h->Z, nzones, nlayers, zone_of_cell, err, nranks, rank, zone_begin)) { h_err = err; return SWE_ERR_ARG; }
+    h->zones = true;
+    return SWE_OK;
+}
 void swe_host_mesh_free(void* hh) { delete (HostHandle*)hh; }
 
 /* Copies the named array to `out` (capacity in bytes) and returns its element count; out == NULL
@@ -105,6 +115,13 @@ int64_t swe_host_get(void* hh, const char* name, void* out, int64_t cap_bytes) {
         if (n == "link_off") return copy_out(h->Z.link_off, out, cap_bytes);
         if (n == "link_src") return copy_out(h->Z.link_src, out, cap_bytes);
         if (n == "link_dst") return copy_out(h->Z.link_dst, out, cap_bytes);
+        if (n == "zone_rank") return copy_out(h->Z.zone_rank, out, cap_bytes);
+        if (n == "rsend_idx") return copy_out(h->Z.rsend_idx, out, cap_bytes);
+        if (n == "rsend_dst") return copy_out(h->Z.rsend_dst, out, cap_bytes);
+        if (n == "rsend_peer") return copy_out(h->Z.rsend_peer, out, cap_bytes);
+        if (n == "rrecv_idx") return copy_out(h->Z.rrecv_idx, out, cap_bytes);
+        if (n == "rsend_off") return copy_out(h->Z.rsend_off, out, cap_bytes);
+        if (n == "rrecv_off") return copy_out(h->Z.rrecv_off, out, cap_bytes);
         if (n == "zone_offset" || n == "zone_nowned" || n == "zone_ncells") {
             std::vector<int64_t> v;
             for (const ZoneDesc& zd : h->Z.z)

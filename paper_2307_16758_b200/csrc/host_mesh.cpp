@@ -326,13 +326,24 @@ void rcb_split(const HostMesh& H, std::vector<int32_t>& ids, int z0, int nz, std
 }  // namespace
 
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32_t* zone_of_cell_user,
-                 std::string& err) {
+                 std::string& err, int nranks, int rank, const int32_t* zone_begin) {
     const MeshArrays& G = H.m;
     const int64_t nc = G.nc;
     Z = ZoneSet();
     if (nz < 1) { err = "nzones must be >= 1"; return false; }
     if (nlayers < 1 || nlayers > 3) { err = "nlayers must be 1, 2 or 3"; return false; }
     Z.nz = nz; Z.nlayers = nlayers;
+    if (nranks < 1 || rank < 0 || rank >= nranks) { err = "bad rank / nranks"; return false; }
+    Z.nranks = nranks; Z.rank = rank;
+    Z.zone_rank.assign(nz, 0);
+    if (nranks > 1) {
+        if (!zone_begin || zone_begin[0] != 0 || zone_begin[nranks] != nz) { err = "zone_begin must run from 0 to nzones"; return false; }
+        for (int r = 0; r < nranks; ++r) {
+            if (zone_begin[r + 1] < zone_begin[r]) { err = "zone_begin must be non-decreasing"; return false; }
+            for (int zi = zone_begin[r]; zi < zone_begin[r + 1]; ++zi) Z.zone_rank[zi] = r;
+        }
+    }
+    auto resident = [&](int zi) { return Z.zone_rank[zi] == rank; };
     Z.zone_of.assign(nc, -1);
     if (zone_of_cell_user) {
         for (int64_t i = 0; i < nc; ++i) {
@@ -391,9 +402,16 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             zd.layer.push_back(gq.layer);
         }
     }
-    int64_t off = 0;
-    for (ZoneDesc& zd : Z.z) { zd.offset = off; off += (int64_t)zd.cells.size(); }
-    const int64_t ncz = off;
+    // offset of every zone in the concatenated mesh of the rank that holds it
+    std::vector<int64_t> owner_off(nz, 0), rank_cells(nranks, 0);
+    for (int zi = 0; zi < nz; ++zi) {
+        owner_off[zi] = rank_cells[Z.zone_rank[zi]];
+        rank_cells[Z.zone_rank[zi]] += (int64_t)Z.z[zi].cells.size();
+        Z.z[zi].offset = resident(zi) ? owner_off[zi] : -1;
+    }
+    const int64_t ncz = rank_cells[rank];
+    for (int r = 0; r < nranks; ++r)
+        if (rank_cells[r] > (int64_t)INT32_MAX / 4) { err = "zoned mesh too large"; return false; }
     if (ncz > (int64_t)INT32_MAX / 4) { err = "zoned mesh too large"; return false; }
 
     // ---- concatenated zoned mesh ----
@@ -408,6 +426,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     std::vector<int32_t> emark(G.ne, -1);
     std::vector<std::vector<int32_t>> zint(nz), zbnd(nz);   // global edge ids per zone
     for (int zi = 0; zi < nz; ++zi) {
+        if (!resident(zi)) continue;
         ZoneDesc& zd = Z.z[zi];
         for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = (int32_t)j;
         // interior edges touching an owned cell, in the order the owned cells meet them
@@ -441,6 +460,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     M.btag.assign(M.ne - M.ne_int, -1);
     std::vector<int32_t> eloc(G.ne, -1);
     for (int zi = 0; zi < nz; ++zi) {
+        if (!resident(zi)) continue;
         ZoneDesc& zd = Z.z[zi];
         const int64_t o = zd.offset;
         for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = (int32_t)j;
@@ -486,10 +506,12 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         }
         for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = -1;
     }
-    // ---- flattened exchange lists ----
+    // ---- flattened exchange lists: links between two resident zones ----
     Z.link_off.push_back(0);
-    for (int zi = 0; zi < nz; ++zi)
+    for (int zi = 0; zi < nz; ++zi) {
+        if (!resident(zi)) continue;
         for (const ZoneLink& lk : Z.z[zi].links) {
+            if (!resident(lk.src)) continue;
             for (int32_t j = 0; j < lk.count; ++j) {
                 Z.send_idx.push_back((int32_t)(Z.z[lk.src].offset + lk.send[j]));
                 Z.recv_idx.push_back((int32_t)(Z.z[zi].offset + lk.start + j));
@@ -498,6 +520,27 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             Z.link_src.push_back(lk.src);
             Z.link_dst.push_back(zi);
         }
+    }
+    // ---- links that cross ranks, grouped by peer, ordered by (destination zone, source zone) ----
+    Z.rsend_off.assign(nranks + 1, 0);
+    Z.rrecv_off.assign(nranks + 1, 0);
+    for (int p = 0; p < nranks; ++p) {
+        if (p != rank)
+            for (int zi = 0; zi < nz; ++zi)
+                for (const ZoneLink& lk : Z.z[zi].links) {
+                    if (Z.zone_rank[zi] == p && resident(lk.src))          // we own the source
+                        for (int32_t j = 0; j < lk.count; ++j) {
+                            Z.rsend_idx.push_back((int32_t)(Z.z[lk.src].offset + lk.send[j]));
+                            Z.rsend_dst.push_back((int32_t)(owner_off[zi] + lk.start + j));
+                            Z.rsend_peer.push_back(p);
+                        }
+                    if (resident(zi) && Z.zone_rank[lk.src] == p)          // we own the ghost
+                        for (int32_t j = 0; j < lk.count; ++j)
+                            Z.rrecv_idx.push_back((int32_t)(Z.z[zi].offset + lk.start + j));
+                }
+        Z.rsend_off[p + 1] = (int64_t)Z.rsend_idx.size();
+        Z.rrecv_off[p + 1] = (int64_t)Z.rrecv_idx.size();
+    }
     return true;
 }
 

@@ -56,6 +56,17 @@ struct ZoneSet {
     std::vector<int32_t> recv_idx;           // concatenated-mesh index of the ghost it lands in
     std::vector<int64_t> link_off;           // offsets into send_idx per link (+ total)
     std::vector<int32_t> link_src, link_dst; // zone ids per link
+    // distribution over ranks (scope row f3): zones [zone_begin[r], zone_begin[r+1]) live on rank r.
+    // Only this rank's zones are in `mesh`; links between two resident zones are in the lists
+    // above; links that cross ranks are here, grouped by peer rank and, inside a peer, ordered by
+    // (destination zone, source zone) -- the order both ends derive independently.
+    int nranks = 1, rank = 0;
+    std::vector<int32_t> zone_rank;          // owner rank per zone
+    std::vector<int32_t> rsend_idx;          // resident cells packed for remote ghosts
+    std::vector<int32_t> rsend_dst;          // where each of them lands: ghost index in the PEER's numbering
+    std::vector<int32_t> rsend_peer;         // and the peer rank (for the one-kernel push over peer memory)
+    std::vector<int32_t> rrecv_idx;          // resident ghost cells filled from remote owners
+    std::vector<int64_t> rsend_off, rrecv_off;   // nranks + 1 each
 };
 
 struct HostMesh {
@@ -76,6 +87,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
 // Builds the zone decomposition and the concatenated zoned mesh.  zone_of_cell_user may be null
 // (recursive coordinate bisection).  Returns false and sets err on invalid arguments.
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nzones, int nlayers,
-                 const int32_t* zone_of_cell_user, std::string& err);
+                 const int32_t* zone_of_cell_user, std::string& err, int nranks = 1, int rank = 0,
+                 const int32_t* zone_begin = nullptr);
 
 }  // namespace swe

@@ -75,6 +75,7 @@ struct swe_ctx {
     double beta = 1.0;
     std::map<int, std::pair<int, double>> bc;
     StepScalars* d_S = nullptr;
+    int* d_flag = nullptr;             // validation flag of swe_set_state
     bool min_valid = false;
     int64_t launches = 0, halo_bytes = 0, steps = 0;
     // zone exchange
@@ -83,6 +84,15 @@ struct swe_ctx {
     int* d_src_of_cell = nullptr;
     double* d_sendbuf = nullptr;
     int64_t nsend = 0;
+    int* d_rsend_idx = nullptr;        // links that cross ranks (swe_zones_create_dist)
+    int* d_rrecv_idx = nullptr;
+    int64_t nrsend = 0, nrrecv = 0;
+    int* d_rsend_dst = nullptr;        // push over peer memory: ghost index on the peer, peer rank,
+    int* d_rsend_peer = nullptr;       // and the peers' two state buffers (device arrays of nranks pointers)
+    double4** d_peerA = nullptr;
+    double4** d_peerB = nullptr;
+    std::vector<void*> peerA, peerB;   // host copies; [rank] = this context's own buffers
+    std::vector<char> peer_ipc;        // 1: opened with cudaIpcOpenMemHandle (closed in free_zones)
     // staging for host pointers
     double* d_stage = nullptr;
     size_t stage_elems = 0;
@@ -247,6 +257,18 @@ void free_zones(swe_ctx* c) {
     if (c->d_recv_idx) cudaFree(c->d_recv_idx);
     if (c->d_src_of_cell) cudaFree(c->d_src_of_cell);
     if (c->d_sendbuf) cudaFree(c->d_sendbuf);
+    if (c->d_rsend_idx) cudaFree(c->d_rsend_idx);
+    if (c->d_rrecv_idx) cudaFree(c->d_rrecv_idx);
+    if (c->d_rsend_dst) cudaFree(c->d_rsend_dst);
+    if (c->d_rsend_peer) cudaFree(c->d_rsend_peer);
+    if (c->d_peerA) cudaFree(c->d_peerA);
+    if (c->d_peerB) cudaFree(c->d_peerB);
+    for (size_t p = 0; p < c->peer_ipc.size(); ++p)
+        if (c->peer_ipc[p]) { cudaIpcCloseMemHandle(c->peerA[p]); cudaIpcCloseMemHandle(c->peerB[p]); }
+    c->peerA.clear(); c->peerB.clear(); c->peer_ipc.clear();
+    c->d_rsend_idx = c->d_rrecv_idx = c->d_rsend_dst = c->d_rsend_peer = nullptr;
+    c->d_peerA = c->d_peerB = nullptr;
+    c->nrsend = c->nrrecv = 0;
     c->d_send_idx = c->d_recv_idx = c->d_src_of_cell = nullptr;
     c->d_sendbuf = nullptr;
     c->nsend = 0;
@@ -390,6 +412,7 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
         cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&c->d_flag, sizeof(int));
         if (e != cudaSuccess) rc = fail(SWE_ERR_CUDA, cudaGetErrorString(e));
     }
     if (rc == SWE_OK) {
@@ -420,6 +443,7 @@ int swe_mesh_destroy(swe_ctx* c) {
     free_zones(c);
     c->g.release();
     if (c->d_S) cudaFree(c->d_S);
+    if (c->d_flag) cudaFree(c->d_flag);
     if (c->d_stage) cudaFree(c->d_stage);
     delete c;
     return SWE_OK;
@@ -489,14 +513,12 @@ int swe_set_state(swe_ctx* c, const double* h, const double* hu, const double* h
         CU(cudaMemcpyAsync(c->d_stage + 2 * nt, hv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
         dh = c->d_stage; dhu = c->d_stage + nt; dhv = c->d_stage + 2 * nt;
     }
-    int* flag = nullptr;
-    CU(cudaMalloc((void**)&flag, sizeof(int)));
-    cudaMemsetAsync(flag, 0, sizeof(int), c->stream);
+    int* flag = c->d_flag;
+    CU(cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
     k_check_state<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(dh, nt, flag);
     int bad = 0;
     cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
     cudaError_t e = cudaStreamSynchronize(c->stream);
-    cudaFree(flag);
     if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
     if (bad) return fail(SWE_ERR_STATE, "h contains NaN or a negative depth");
     k_state_from_user<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(c->g.A, c->g.d_cell_user, c->g.dm.zc, dh, dhu, dhv, (int)nt);
@@ -546,6 +568,8 @@ int swe_set_time(swe_ctx* c, double t) {
 int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (nsteps < 0 || !(cfl > 0.0) || scheme < 0 || scheme > 3) return fail(SWE_ERR_ARG, "bad step arguments");
+    if (c->has_zones && c->Z.nranks > 1)
+        return fail(SWE_ERR_STATE, "zones are distributed over ranks: drive the step with swe_dist_* / swe_halo_*");
     if (c->has_zones && (scheme == K_WAF || scheme == K_MUSCL_MS) && c->Z.nlayers < 2)
         return fail(SWE_ERR_STATE, "WAF and the multislope MUSCL need zones with at least 2 ghost layers");
     Store& st = c->active();
@@ -724,7 +748,8 @@ int swe_get_stats(const swe_ctx* c, int64_t* steps, int64_t* kernel_launches, in
 }
 
 // ---- zones ----
-int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell) {
+static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell, int nranks,
+                             int rank, const int32_t* zone_begin) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (nzones < 0) return fail(SWE_ERR_ARG, "nzones must be >= 0");
     int rc = sync_global_from_zoned(c); if (rc) return rc;
@@ -741,7 +766,7 @@ int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of
     }
     std::string err;
     bool ok = false;
-    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err); }
+    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err, nranks, rank, zone_begin); }
     catch (const std::bad_alloc&) { c->Z = ZoneSet(); return fail(SWE_ERR_NOMEM, "out of host memory in zone set-up"); }
     if (!ok) { c->Z = ZoneSet(); return fail(SWE_ERR_ARG, err); }
     rc = upload_store(c, c->z, c->Z.mesh);
@@ -765,6 +790,22 @@ int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of
         CU(cudaMemcpyAsync(c->d_recv_idx, c->Z.recv_idx.data(), c->nsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     }
     CU(cudaMemcpyAsync(c->d_src_of_cell, c->Z.src_of_cell.data(), (size_t)c->z.nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    c->nrsend = (int64_t)c->Z.rsend_idx.size();
+    c->nrrecv = (int64_t)c->Z.rrecv_idx.size();
+    CU(cudaMalloc((void**)&c->d_rsend_idx, (size_t)(c->nrsend ? c->nrsend : 1) * sizeof(int)));
+    CU(cudaMalloc((void**)&c->d_rrecv_idx, (size_t)(c->nrrecv ? c->nrrecv : 1) * sizeof(int)));
+    if (c->nrsend) CU(cudaMemcpyAsync(c->d_rsend_idx, c->Z.rsend_idx.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    if (c->nrrecv) CU(cudaMemcpyAsync(c->d_rrecv_idx, c->Z.rrecv_idx.data(), c->nrrecv * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMalloc((void**)&c->d_rsend_dst, (size_t)(c->nrsend ? c->nrsend : 1) * sizeof(int)));
+    CU(cudaMalloc((void**)&c->d_rsend_peer, (size_t)(c->nrsend ? c->nrsend : 1) * sizeof(int)));
+    if (c->nrsend) {
+        CU(cudaMemcpyAsync(c->d_rsend_dst, c->Z.rsend_dst.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_rsend_peer, c->Z.rsend_peer.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    }
+    CU(cudaMalloc((void**)&c->d_peerA, (size_t)nranks * sizeof(double4*)));
+    CU(cudaMalloc((void**)&c->d_peerB, (size_t)nranks * sizeof(double4*)));
+    c->peerA.assign(nranks, nullptr); c->peerB.assign(nranks, nullptr); c->peer_ipc.assign(nranks, 0);
+    c->peerA[rank] = c->z.A; c->peerB[rank] = c->z.B;
     c->has_zones = true;
     rc = refresh_bc(c, c->z); if (rc) return rc;
     k_gather_cells<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.A, c->g.A, c->d_src_of_cell, (int)c->z.nc);
@@ -774,6 +815,189 @@ int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of
     CU(cudaStreamSynchronize(c->stream));
     // the host copies of the big zoned arrays are no longer needed
     c->Z.mesh = MeshArrays();
+    return SWE_OK;
+}
+
+int swe_zones_create(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell) {
+    return zones_create_impl(c, nzones, nlayers, zone_of_cell, 1, 0, nullptr);
+}
+
+// ---- zones distributed over ranks (scope row f3): the caller moves the halo buffers ----
+int swe_zones_create_dist(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell, int nranks,
+                          int rank, const int32_t* zone_begin) {
+    if (nzones < 1 || nranks < 1 || rank < 0 || rank >= nranks || (nranks > 1 && !zone_begin))
+        return fail(SWE_ERR_ARG, "bad distributed zone arguments");
+    return zones_create_impl(c, nzones, nlayers, zone_of_cell, nranks, rank, zone_begin);
+}
+
+int swe_halo_counts(const swe_ctx* c, int64_t* send_cells, int64_t* recv_cells) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    for (int p = 0; p < c->Z.nranks; ++p) {
+        if (send_cells) send_cells[p] = c->Z.rsend_off[p + 1] - c->Z.rsend_off[p];
+        if (recv_cells) recv_cells[p] = c->Z.rrecv_off[p + 1] - c->Z.rrecv_off[p];
+    }
+    return SWE_OK;
+}
+
+int swe_halo_pack(swe_ctx* c, int buffer, double* sendbuf) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (buffer < 0 || buffer > 1 || (c->nrsend && (!sendbuf || !is_device_ptr(sendbuf)))) return fail(SWE_ERR_ARG, "bad halo buffer");
+    if (c->nrsend) {
+        launch(c, KIND_PACK, [&] {
+            k_pack_state<<<grid_for(c->nrsend, c->grid_light), 256, 0, c->stream>>>(buffer ? c->z.B : c->z.A, c->d_rsend_idx, sendbuf, 0, c->nrsend);
+        });
+        c->halo_bytes += c->nrsend * (4 + 32 + 24);
+    }
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_halo_unpack(swe_ctx* c, int buffer, const double* recvbuf) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (buffer < 0 || buffer > 1 || (c->nrrecv && (!recvbuf || !is_device_ptr(recvbuf)))) return fail(SWE_ERR_ARG, "bad halo buffer");
+    if (c->nrrecv) {
+        launch(c, KIND_UNPACK, [&] {
+            k_unpack_state<<<grid_for(c->nrrecv, c->grid_light), 256, 0, c->stream>>>(buffer ? c->z.B : c->z.A, c->d_rrecv_idx, recvbuf, c->z.dm.zc, 0, c->nrrecv);
+        });
+        c->halo_bytes += c->nrrecv * (4 + 24 + 8 + 32);
+    }
+    run_exchange_state(c, buffer ? c->z.B : c->z.A, 0, c->nsend, true, true);    // links between resident zones
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+// ---- halo exchange as one kernel over peer memory ----
+static int peer_store(swe_ctx* c, int peer, void* A, void* B, bool ipc) {
+    if (c->peer_ipc[peer]) { cudaIpcCloseMemHandle(c->peerA[peer]); cudaIpcCloseMemHandle(c->peerB[peer]); }
+    c->peerA[peer] = A; c->peerB[peer] = B; c->peer_ipc[peer] = ipc ? 1 : 0;
+    return SWE_OK;
+}
+static int peer_upload(swe_ctx* c) {
+    const size_t n = c->peerA.size();
+    CU(cudaMemcpyAsync(c->d_peerA, c->peerA.data(), n * sizeof(void*), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->d_peerB, c->peerB.data(), n * sizeof(void*), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+static int check_peer(swe_ctx* c, int peer) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (peer < 0 || peer >= c->Z.nranks || peer == c->Z.rank) return fail(SWE_ERR_ARG, "peer must be another rank");
+    return SWE_OK;
+}
+
+int swe_peer_export(swe_ctx* c, unsigned char* handles) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (!handles) return fail(SWE_ERR_ARG, "NULL handle buffer");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, c->z.A));
+    std::memcpy(handles, &h, 64);
+    CU(cudaIpcGetMemHandle(&h, c->z.B));
+    std::memcpy(handles + 64, &h, 64);
+    return SWE_OK;
+}
+
+int swe_peer_import(swe_ctx* c, int peer, const unsigned char* handles) {
+    int rc = check_peer(c, peer); if (rc) return rc;
+    if (!handles) return fail(SWE_ERR_ARG, "NULL handle buffer");
+    cudaIpcMemHandle_t h;
+    void *A = nullptr, *B = nullptr;
+    std::memcpy(&h, handles, 64);
+    CU(cudaIpcOpenMemHandle(&A, h, cudaIpcMemLazyEnablePeerAccess));
+    std::memcpy(&h, handles + 64, 64);
+    cudaError_t e = cudaIpcOpenMemHandle(&B, h, cudaIpcMemLazyEnablePeerAccess);
+    if (e != cudaSuccess) { cudaIpcCloseMemHandle(A); return fail(SWE_ERR_CUDA, cudaGetErrorString(e)); }
+    peer_store(c, peer, A, B, true);
+    return peer_upload(c);
+}
+
+int swe_peer_raw(swe_ctx* c, void** A, void** B) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (A) *A = c->z.A;
+    if (B) *B = c->z.B;
+    return SWE_OK;
+}
+
+int swe_peer_set_raw(swe_ctx* c, int peer, void* A, void* B) {
+    int rc = check_peer(c, peer); if (rc) return rc;
+    if (!A || !B || !is_device_ptr(A) || !is_device_ptr(B)) return fail(SWE_ERR_ARG, "peer buffers must be device pointers");
+    peer_store(c, peer, A, B, false);
+    return peer_upload(c);
+}
+
+int swe_halo_push(swe_ctx* c, int buffer) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (buffer < 0 || buffer > 1) return fail(SWE_ERR_ARG, "bad halo buffer");
+    for (int p = 0; p < c->Z.nranks; ++p)
+        if (c->Z.rsend_off[p + 1] > c->Z.rsend_off[p] && !c->peerA[p])
+            return fail(SWE_ERR_STATE, "swe_halo_push: a peer this rank sends to has not been imported");
+    double4* U = buffer ? c->z.B : c->z.A;
+    if (c->nrsend) {
+        launch(c, KIND_PACK, [&] {
+            k_halo_push<<<grid_for(c->nrsend, c->grid_light), 256, 0, c->stream>>>(U, c->d_rsend_idx, c->d_rsend_dst, c->d_rsend_peer,
+                                                                                  buffer ? c->d_peerB : c->d_peerA, c->nrsend);
+        });
+        c->halo_bytes += c->nrsend * (12 + 32 + 32);
+    }
+    run_exchange_state(c, U, 0, c->nsend, true, true);    // links between resident zones
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_dist_local_min(swe_ctx* c, double* min_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!min_out || !is_device_ptr(min_out)) return fail(SWE_ERR_ARG, "min_out must be a device pointer");
+    Store& st = c->active();
+    if (!c->min_valid) run_dt_reduce(c, st, st.A);
+    c->min_valid = true;
+    CU(cudaMemcpyAsync(min_out, &c->d_S->min_bits, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return SWE_OK;
+}
+
+int swe_dist_begin_step(swe_ctx* c, const double* min_in, double cfl) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!min_in || !is_device_ptr(min_in) || !(cfl > 0.0)) return fail(SWE_ERR_ARG, "bad arguments");
+    CU(cudaMemcpyAsync(&c->d_S->min_bits, min_in, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    launch(c, KIND_MISC, [&] { k_dt_finalize<<<1, 1, 0, c->stream>>>(c->d_S, cfl, 1); });
+    c->min_valid = false;
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_dist_stage(swe_ctx* c, int scheme, int stage) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (scheme < 0 || scheme > 3 || stage < 0 || stage > 1) return fail(SWE_ERR_ARG, "bad stage arguments");
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (scheme != K_HLLC && c->Z.nlayers < 2)
+        return fail(SWE_ERR_STATE, "distributed MUSCL / WAF stages need zones with at least 2 ghost layers");
+    const bool heun = scheme == K_MUSCL || scheme == K_MUSCL_MS;
+    if (!heun && stage != 0) return fail(SWE_ERR_ARG, "Euler schemes have one stage");
+    Store& st = c->z;
+    const double4* Uin = (stage == 0) ? st.A : st.B;
+    if (scheme == K_MUSCL) run_grad(c, st, Uin);
+    run_flux(c, st, Uin, scheme);
+    if (heun && stage == 0) run_update(c, st, st.A, nullptr, st.B, 0, false);
+    else if (heun) run_update(c, st, st.B, st.A, st.A, 1, true);
+    else run_update(c, st, st.A, nullptr, st.A, 0, true);
+    if (!heun || stage == 1) { c->min_valid = true; c->steps++; }
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_get_time(swe_ctx* c, double* t_out, double* last_dt_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    StepScalars hs;
+    CU(cudaMemcpyAsync(&hs, c->d_S, sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (t_out) *t_out = hs.t;
+    if (last_dt_out) *last_dt_out = hs.last_dt;
     return SWE_OK;
 }
 
@@ -800,7 +1024,7 @@ int swe_zone_stats(const swe_ctx* c, int64_t* send_cells_total, int64_t* bytes_p
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
     int64_t gh = 0;
-    for (const ZoneDesc& zd : c->Z.z) gh += (int64_t)zd.cells.size() - zd.nowned;
+    for (const ZoneDesc& zd : c->Z.z) if (zd.offset >= 0) gh += (int64_t)zd.cells.size() - zd.nowned;
     if (send_cells_total) *send_cells_total = c->nsend;
     if (bytes_per_exchange) *bytes_per_exchange = c->nsend * 24;
     if (ghost_cells_total) *ghost_cells_total = gh;

@@ -1,9 +1,20 @@
-"""Multi-process plumbing for bench.py (one process per GPU, torch.distributed).
+"""Multi-process driver (one process per GPU, torch.distributed) -- SURVEY.md 8(e), scope row f3.
 
-The time step on one GPU has no data-path collective; with N > 1 ranks bench.py runs N independent
-replicas ("replicas only", DESIGN.md section 'Multi-GPU') and only the timing is reduced: barrier
-before and after the timed region, MAX of the per-rank device times, SUM of the units processed.
-Backend: nccl when CUDA is available, else gloo (CPU tests, world_size 2).
+The explicit step has ONE real exchange per stage (the ghost cells of U) plus one
+scalar min for dt per step.  `DistSolver` holds this rank's zones of a decomposition every rank
+derives from the same mesh and drives the C-ABI calls of include/swe_b200.h ("zones distributed
+over ranks"); the library never calls a communication library, this module does, and only for
+
+  * the 8-byte all-reduce(min) of dt (which doubles as the stream-ordered barrier that orders the
+    peer-memory pushes) and one more barrier per step,
+  * with transport "staged": an all-to-all of the packed halo buffers (pack -> NCCL -> unpack),
+  * set-up: the all-gather of the CUDA IPC handles of the state buffers (transport "p2p": the
+    exchange is then ONE kernel per rank storing its send cells straight into its peers' ghost
+    ranges over NVLink / NVSwitch).
+
+Backend: nccl when CUDA is available (gloo with SWE_DIST_GLOO=1 or on CPU: tests).  With gloo,
+CUDA tensors are staged through the host (test configurations only: 2 processes sharing one GPU).
+Everything else here is bench.py plumbing: barrier, max-over-ranks time, sums, block sharding.
 """
 import os
 
@@ -17,11 +28,11 @@ def init_from_env():
         import torch
         import torch.distributed as dist
         if not dist.is_initialized():
-            backend = "nccl" if torch.cuda.is_available() else "gloo"
+            backend = "nccl" if torch.cuda.is_available() and not os.environ.get("SWE_DIST_GLOO") else "gloo"
             os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
             os.environ.setdefault("MASTER_PORT", "29511")
-            if backend == "nccl":
-                torch.cuda.set_device(local)
+            if torch.cuda.is_available():
+                torch.cuda.set_device(local % torch.cuda.device_count())
             dist.init_process_group(backend=backend, rank=rank, world_size=world)
     return rank, world, local
 
@@ -70,3 +81,164 @@ def shard_units(n_units, rank, world):
     base, rem = divmod(int(n_units), int(world))
     lo = rank * base + min(rank, rem)
     return lo, lo + base + (1 if rank < rem else 0)
+
+
+def zone_blocks(nzones, world):
+    """zone_begin of swe_zones_create_dist: contiguous blocks of zones per rank."""
+    return [shard_units(nzones, r, world)[0] for r in range(world)] + [int(nzones)]
+
+
+class TorchComm:
+    """The collectives DistSolver needs, over torch.distributed (nccl; gloo stages CUDA tensors
+    through the host).  All calls are collective over the default group."""
+
+    def __init__(self):
+        import torch.distributed as dist
+        self.dist = dist
+        self.rank, self.world = dist.get_rank(), dist.get_world_size()
+        self.staged_host = dist.get_backend() != "nccl"
+
+    def allreduce_min(self, t):
+        """In-place MIN all-reduce of a device tensor, ordered on the current stream."""
+        if self.staged_host and t.is_cuda:
+            c = t.cpu()
+            self.dist.all_reduce(c, op=self.dist.ReduceOp.MIN)
+            t.copy_(c)
+        else:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
+
+    def all_to_all(self, recv, send, recv_splits, send_splits):
+        if self.staged_host and send.is_cuda:
+            r = recv.cpu()
+            self.dist.all_to_all_single(r, send.cpu(), recv_splits, send_splits)
+            recv.copy_(r)
+        else:
+            self.dist.all_to_all_single(recv, send, recv_splits, send_splits)
+
+    def all_gather_bytes(self, arr):
+        """arr: numpy uint8; returns the list of every rank's array."""
+        import torch
+        t = torch.from_numpy(arr.copy())
+        if not self.staged_host:
+            t = t.cuda()
+        out = [torch.empty_like(t) for _ in range(self.world)]
+        self.dist.all_gather(out, t)
+        return [o.cpu().numpy() for o in out]
+
+    def allreduce_sum(self, t):
+        if self.staged_host and t.is_cuda:
+            c = t.cpu()
+            self.dist.all_reduce(c, op=self.dist.ReduceOp.SUM)
+            t.copy_(c)
+        else:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+
+    def host_barrier(self):
+        import torch
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()
+        self.dist.barrier()
+
+
+class DistSolver:
+    """This rank's share of a mesh split into zones over the ranks of the default process group.
+
+    cfg: an input dictionary of swe_inputs.configs (every rank passes the same one); nzones zones by
+    recursive coordinate bisection (or zone_of_cell), rank r holding the block zone_blocks()[r:r+2];
+    nlayers ghost layers (>= 2 for MUSCL / WAF / MUSCL_MS); transport "p2p" (peer-memory push, one
+    kernel per exchange) or "staged" (pack -> all-to-all -> unpack).
+    """
+
+    def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None):
+        import torch
+        from . import binding as sw
+        self.sw, self.torch = sw, torch
+        self.comm = comm if comm is not None else TorchComm()
+        self.rank, self.world = self.comm.rank, self.comm.world
+        if transport not in ("p2p", "staged"):
+            raise ValueError("transport must be 'p2p' or 'staged'")
+        self.transport = transport
+        if nzones is None:
+            nzones = 1
+            while nzones < self.world:
+                nzones *= 2
+        self.nzones, self.nlayers = int(nzones), int(nlayers)
+        self.ctx = sw.create_from_config(cfg)
+        self.ncell = sw.swe_mesh_info(self.ctx)["ncell"]
+        sw.swe_zones_create_dist(self.ctx, self.nzones, self.nlayers, zone_of_cell, self.world, self.rank,
+                                 zone_blocks(self.nzones, self.world))
+        self.send_cells, self.recv_cells = sw.swe_halo_counts(self.ctx, self.world)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.minbuf = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.token = torch.zeros(1, dtype=torch.float64, device=dev)
+        if transport == "staged":
+            self.sendbuf = torch.zeros(max(1, 3 * int(self.send_cells.sum())), dtype=torch.float64, device=dev)
+            self.recvbuf = torch.zeros(max(1, 3 * int(self.recv_cells.sum())), dtype=torch.float64, device=dev)
+            self.ssplit = [3 * int(v) for v in self.send_cells]
+            self.rsplit = [3 * int(v) for v in self.recv_cells]
+        else:
+            handles = self.comm.all_gather_bytes(sw.swe_peer_export(self.ctx))
+            for p in range(self.world):
+                if p != self.rank:
+                    sw.swe_peer_import(self.ctx, p, handles[p])
+        self.comm.host_barrier()
+
+    # -- one exchange of the ghosts of state buffer `buffer` (0 = U, 1 = the Heun stage buffer) --
+    def exchange(self, buffer):
+        sw = self.sw
+        if self.transport == "p2p":
+            sw.swe_halo_push(self.ctx, buffer)
+        else:
+            sw.swe_halo_pack(self.ctx, buffer, self.sendbuf)
+            n_s, n_r = sum(self.ssplit), sum(self.rsplit)
+            self.comm.all_to_all(self.recvbuf[:n_r], self.sendbuf[:n_s], self.rsplit, self.ssplit)
+            sw.swe_halo_unpack(self.ctx, buffer, self.recvbuf)
+
+    def barrier_stream(self):
+        """Stream-ordered barrier: nobody's stream passes it before everybody's reached it."""
+        self.comm.allreduce_min(self.token)
+
+    def step(self, nsteps, cfl, scheme):
+        """nsteps time steps, asynchronous on the current stream (nccl)."""
+        sw = self.sw
+        sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
+        heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
+        p2p = self.transport == "p2p"
+        for _ in range(int(nsteps)):
+            self.exchange(0)
+            sw.swe_dist_local_min(self.ctx, self.minbuf)
+            self.comm.allreduce_min(self.minbuf)       # dt; with p2p also: every push of buffer 0 has landed
+            sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+            sw.swe_dist_stage(self.ctx, sch, 0)
+            if heun:
+                self.exchange(1)
+                if p2p:
+                    self.barrier_stream()              # every push of buffer 1 has landed
+                sw.swe_dist_stage(self.ctx, sch, 1)
+            elif p2p:
+                self.barrier_stream()                  # everybody has read its ghosts of buffer 0
+
+    def time(self):
+        return self.sw.swe_get_time(self.ctx)
+
+    def set_state(self, h, hu, hv):
+        self.comm.host_barrier()
+        self.sw.swe_set_state(self.ctx, h, hu, hv)
+        self.comm.host_barrier()
+
+    def get_state_local(self, h, hu, hv):
+        """Fills the entries of this rank's owned cells only."""
+        self.sw.swe_get_state(self.ctx, h, hu, hv)
+
+    def get_state(self):
+        """The full state on every rank (numpy): owned cells of all ranks summed over zero arrays."""
+        torch = self.torch
+        out = torch.zeros(3, self.ncell, dtype=torch.float64, device=self.minbuf.device)
+        self.sw.swe_get_state(self.ctx, out[0], out[1], out[2])
+        self.comm.allreduce_sum(out)
+        return tuple(o.cpu().numpy() for o in out)
+
+    def close(self):
+        self.comm.host_barrier()                       # nobody still pushes into this rank's buffers
+        self.sw.swe_mesh_destroy(self.ctx)
+        self.ctx = None

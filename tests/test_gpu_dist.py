@@ -1,0 +1,201 @@
+"""Multi-GPU driver (scope row f3) on ONE GPU: the ranks' kernels never wait on one
+another, so the path can be run rank after rank.
+
+ * in-process: `world` contexts in one process stand for the ranks; every phase of dist.DistSolver's
+   step (push / pack-transfer-unpack, min-reduce, stages) is run for all ranks in turn, the
+   "transfer" being a device copy between the ranks' halo buffers.  The result must be BIT-identical
+   to the un-zoned run for every scheme, both transports, 1..3 zones per rank.
+ * two processes sharing cuda:0 over gloo (host-staged collectives, CUDA IPC between the
+   processes): dist.DistSolver itself, the code bench.py runs at N > 1.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.multiprocessing as mp
+
+import paper_2307_16758_b200 as sw
+from paper_2307_16758_b200 import dist as swdist
+from swe_inputs import config3
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _river():
+    return config3(length=3200.0, half_width=600.0, w2=30.0, n4=4, n8=3)
+
+
+class _Ranks:
+    """`world` ranks as contexts of one process."""
+
+    def __init__(self, cfg, world, nz, nl, transport):
+        self.world, self.transport = world, transport
+        self.ctx = [sw.create_from_config(cfg) for _ in range(world)]
+        blocks = swdist.zone_blocks(nz, world)
+        for r, c in enumerate(self.ctx):
+            sw.swe_zones_create_dist(c, nz, nl, None, world, r, blocks)
+        self.counts = [sw.swe_halo_counts(c, world) for c in self.ctx]
+        dev = torch.device("cuda")
+        self.mins = torch.zeros(world, dtype=torch.float64, device=dev)
+        if transport == "p2p":
+            raw = [sw.swe_peer_raw(c) for c in self.ctx]
+            for r, c in enumerate(self.ctx):
+                for p in range(world):
+                    if p != r:
+                        sw.swe_peer_set_raw(c, p, *raw[p])
+        else:
+            self.sendbuf = [torch.zeros(max(1, 3 * int(s.sum())), dtype=torch.float64, device=dev) for s, _ in self.counts]
+            self.recvbuf = [torch.full((max(1, 3 * int(r.sum())),), np.nan, dtype=torch.float64, device=dev) for _, r in self.counts]
+
+    def exchange(self, buffer):
+        if self.transport == "p2p":
+            for c in self.ctx:
+                sw.swe_halo_push(c, buffer)
+            return
+        for r, c in enumerate(self.ctx):
+            sw.swe_halo_pack(c, buffer, self.sendbuf[r])
+        soff = [np.concatenate([[0], 3 * np.cumsum(s)]) for s, _ in self.counts]
+        roff = [np.concatenate([[0], 3 * np.cumsum(r)]) for _, r in self.counts]
+        for a in range(self.world):            # the all-to-all
+            for b in range(self.world):
+                n = int(soff[a][b + 1] - soff[a][b])
+                assert n == int(roff[b][a + 1] - roff[b][a])
+                if n:
+                    self.recvbuf[b][int(roff[b][a]):int(roff[b][a]) + n] = self.sendbuf[a][int(soff[a][b]):int(soff[a][b]) + n]
+        for r, c in enumerate(self.ctx):
+            sw.swe_halo_unpack(c, buffer, self.recvbuf[r])
+
+    def step(self, nsteps, cfl, scheme):
+        heun = scheme in ("muscl", "muscl_ms")
+        for _ in range(nsteps):
+            self.exchange(0)
+            for r, c in enumerate(self.ctx):
+                sw.swe_dist_local_min(c, self.mins[r:r + 1])
+            m = self.mins.min().reshape(1)                      # the all-reduce(min)
+            for c in self.ctx:
+                sw.swe_dist_begin_step(c, m, cfl)
+                sw.swe_dist_stage(c, scheme, 0)
+            if heun:
+                self.exchange(1)
+                for c in self.ctx:
+                    sw.swe_dist_stage(c, scheme, 1)
+
+    def state(self, n):
+        out = [np.full(n, np.nan) for _ in range(3)]
+        for c in self.ctx:
+            sw.swe_get_state(c, *out)          # each rank fills the cells it owns
+        return out
+
+    def close(self):
+        torch.cuda.synchronize()
+        for c in self.ctx:
+            sw.swe_mesh_destroy(c)
+
+
+@pytest.mark.parametrize("transport", ["p2p", "staged"])
+@pytest.mark.parametrize("world,nz,nl", [(2, 2, 2), (4, 4, 2), (2, 8, 3), (3, 8, 2)])
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_ranks_in_one_process_bit_identical(transport, world, nz, nl, scheme, cfl):
+    cfg = _river()
+    a = sw.create_from_config(cfg)
+    R = _Ranks(cfg, world, nz, nl, transport)
+    try:
+        n = sw.swe_mesh_info(a)["ncell"]
+        ta = sw.swe_step(a, 30, cfl, scheme)
+        R.step(30, cfl, scheme)
+        ref = sw.swe_get_state(a)
+        got = R.state(n)
+        for x, y in zip(ref, got):
+            assert np.array_equal(x, y)
+        for c in R.ctx:
+            assert sw.swe_get_time(c) == ta
+        # a rank refuses the single-GPU step while its zones are distributed
+        with pytest.raises(sw.SweError) as e:
+            sw.swe_step(R.ctx[0], 1, cfl, scheme)
+        assert e.value.code == sw.SWE_ERR_STATE
+    finally:
+        sw.swe_mesh_destroy(a)
+        R.close()
+
+
+def test_one_layer_hllc_and_errors():
+    cfg = _river()
+    a = sw.create_from_config(cfg)
+    R = _Ranks(cfg, 2, 4, 1, "p2p")
+    try:
+        n = sw.swe_mesh_info(a)["ncell"]
+        sw.swe_step(a, 20, 0.9, "hllc")
+        R.step(20, 0.9, "hllc")
+        for x, y in zip(sw.swe_get_state(a), R.state(n)):
+            assert np.array_equal(x, y)
+        c = R.ctx[0]
+        for bad in (lambda: sw.swe_dist_stage(c, "muscl", 0),        # one ghost layer: HLLC only
+                    lambda: sw.swe_dist_stage(c, "hllc", 1),         # Euler schemes have one stage
+                    lambda: sw.swe_halo_push(c, 2),
+                    lambda: sw.swe_peer_set_raw(c, 0, *sw.swe_peer_raw(c)),     # own rank is not a peer
+                    lambda: sw.swe_halo_pack(c, 0, np.zeros(8)),     # host pointer
+                    lambda: sw.swe_dist_local_min(c, np.zeros(1))):
+            with pytest.raises(sw.SweError):
+                bad()
+        # a rank whose peers were never connected cannot push
+        d = sw.create_from_config(cfg)
+        try:
+            sw.swe_zones_create_dist(d, 4, 1, None, 2, 0, [0, 2, 4])
+            with pytest.raises(sw.SweError) as e:
+                sw.swe_halo_push(d, 0)
+            assert e.value.code == sw.SWE_ERR_STATE
+        finally:
+            sw.swe_mesh_destroy(d)
+    finally:
+        sw.swe_mesh_destroy(a)
+        R.close()
+
+
+def _worker(rank, world, port, transport, scheme, cfl, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port), SWE_DIST_GLOO="1")
+    try:
+        from paper_2307_16758_b200 import dist as d
+        d.init_from_env()
+        cfg = _river()
+        S = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport)
+        S.step(25, cfl, scheme)
+        t = S.time()
+        st = S.get_state()
+        S.close()
+        out = None
+        if rank == 0:
+            a = sw.create_from_config(cfg)
+            ta = sw.swe_step(a, 25, cfl, scheme)
+            ref = sw.swe_get_state(a)
+            sw.swe_mesh_destroy(a)
+            out = bool(ta == t and all(np.array_equal(x, y) for x, y in zip(ref, st)))
+        d.finalize()
+        q.put((rank, out, ""))
+    except Exception as e:       # report instead of hanging the parent
+        import traceback
+        q.put((rank, False, traceback.format_exc() + str(e)))
+
+
+@pytest.mark.parametrize("transport,scheme,cfl", [("p2p", "muscl", 0.45), ("staged", "muscl", 0.45), ("p2p", "hllc", 0.9)])
+def test_two_processes_one_gpu_dist_solver(transport, scheme, cfl):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29700 + os.getpid() % 90
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, transport, scheme, cfl, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    try:
+        res = sorted(q.get(timeout=600) for _ in ps)
+        for p in ps:
+            p.join(120)
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.kill()
+    assert all(r[2] == "" for r in res), [r[2] for r in res]
+    assert res[0][1] is True
