@@ -314,6 +314,7 @@ def main():
     rank, world, local = swdist.init_from_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    local = local % torch.cuda.device_count()      # test configurations put several ranks on one GPU
     torch.cuda.set_device(local)
     sw.lib()   # fails loudly if the CUDA extension is missing
 

@@ -544,6 +544,11 @@ int swe_get_state(const swe_ctx* cc, double* h, double* hu, double* hv) {
     if (!dev) {
         int rc = ensure_stage(c, 3 * (size_t)nt + 2); if (rc) return rc;
         dh = c->d_stage; dhu = c->d_stage + nt; dhv = c->d_stage + 2 * nt;
+        if (c->has_zones && c->Z.nranks > 1) {      // only this rank's cells are written: keep the caller's other entries
+            CU(cudaMemcpyAsync(dh, h, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+            CU(cudaMemcpyAsync(dhu, hu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+            CU(cudaMemcpyAsync(dhv, hv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        }
     }
     Store& st = c->active();
     k_state_to_user<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.A, st.d_cell_user, st.dm.layer, dh, dhu, dhv, (int)st.nc);
