@@ -214,7 +214,7 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
     import paper_2307_16758_b200 as sw
 
     S = swdist.DistSolver(cfg, nzones=args.zones if args.zones > 0 else None, nlayers=args.layers,
-                          transport=args.transport)
+                          transport=args.transport, schedule=args.schedule)
     nt = S.ncell
     info = sw.swe_mesh_info(S.ctx)
     owned = sum(sw.swe_zone_describe_counts(S.ctx, z)[0] for z in range(*swdist.shard_units(S.nzones, rank, world)))
@@ -278,7 +278,8 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
                        "l2": "inputs larger than L2 per rank" if nt / world > 2_000_000 else
                              "a rank's share may fit L2 at this size",
                        "parallelism": "zones over %d ranks (%d zones, %d ghost layers), halo transport %s, "
-                                      "all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport),
+                                      "schedule %s, all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport,
+                                                                              S.schedule),
                        "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": None,
             "gpu_launches": int(launches), "clocks": clocks,
@@ -298,6 +299,7 @@ def main():
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)
     ap.add_argument("--transport", default="p2p", choices=["p2p", "staged"])
+    ap.add_argument("--schedule", default="overlap", choices=["overlap", "plain"])
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)

@@ -173,6 +173,15 @@ int swe_dist_begin_step(swe_ctx* ctx, const double* min_in, double cfl);
  * Euler schemes: updates buffer 0 in place and end the step); stage 1 (Heun only) reads buffer 1
  * and writes U^{n+1} = (U^n + E(U'))/2 to buffer 0.  The ghosts of the buffer read must be current. */
 int swe_dist_stage(swe_ctx* ctx, int scheme, int stage);
+/* The two halves of swe_dist_stage, for the overlap schedule (scope row f2; "high
+ * overlap": the cells of the send lists are updated first, the exchange runs while the rest of the
+ * domain is updated).  swe_dist_flux: gradient + limiter (MUSCL) and edge fluxes of the stage's
+ * input buffer.  swe_dist_update: the cell update of the stage for part 0 = every owned cell,
+ * 1 = only the cells on a send list (remote or resident), 2 = every owned cell but those.  A stage
+ * is flux, then part 0, or flux, part 1, part 2 (in that order: part 2 or 0 of the last stage ends
+ * the step).  The results are bit-identical to swe_dist_stage. */
+int swe_dist_flux(swe_ctx* ctx, int scheme, int stage);
+int swe_dist_update(swe_ctx* ctx, int scheme, int stage, int part);
 /* simulated time and last dt (host pointers; synchronises the stream). */
 int swe_get_time(swe_ctx* ctx, double* t_out, double* last_dt_out);
 
@@ -220,7 +229,8 @@ int swe_host_mesh_build(void** out, int64_t nv, const double* x, const double* y
                         const int32_t* btag, int renumber);
 int swe_host_zones_build(void* handle, int nzones, int nlayers, const int32_t* zone_of_cell);
 /* the distributed variant (swe_zones_create_dist's host half): adds the names "zone_rank",
- * "rsend_idx", "rsend_dst", "rsend_peer", "rrecv_idx", "rsend_off", "rrecv_off" to swe_host_get. */
+ * "rsend_idx", "rsend_dst", "rsend_peer", "rrecv_idx", "rsend_off", "rrecv_off", "send_cells" to
+ * swe_host_get. */
 int swe_host_zones_build_dist(void* handle, int nzones, int nlayers, const int32_t* zone_of_cell,
                               int nranks, int rank, const int32_t* zone_begin);
 void swe_host_mesh_free(void* handle);

@@ -57,6 +57,8 @@ SIGNATURES = {
     "swe_dist_local_min": (C.c_int, [_vp, _vp]),
     "swe_dist_begin_step": (C.c_int, [_vp, _vp, C.c_double]),
     "swe_dist_stage": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "swe_dist_flux": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "swe_dist_update": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int]),
     "swe_get_time": (C.c_int, [_vp, _dp, _dp]),
     "swe_compute_dt": (C.c_int, [_vp, C.c_double, _dp]),
     "swe_gradients": (C.c_int, [_vp, _vp]),
@@ -301,6 +303,14 @@ def swe_dist_stage(ctx, scheme, stage):
     _check(lib().swe_dist_stage(ctx, _scheme(scheme), int(stage)))
 
 
+def swe_dist_flux(ctx, scheme, stage):
+    _check(lib().swe_dist_flux(ctx, _scheme(scheme), int(stage)))
+
+
+def swe_dist_update(ctx, scheme, stage, part=0):
+    _check(lib().swe_dist_update(ctx, _scheme(scheme), int(stage), int(part)))
+
+
 def swe_get_time(ctx):
     t, dt = C.c_double(), C.c_double()
     _check(lib().swe_get_time(ctx, C.byref(t), C.byref(dt)))
@@ -386,7 +396,7 @@ _HOST_DTYPES = {"cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": 
                 "user_cell": np.int32, "zone_of": np.int32, "send_idx": np.int32, "recv_idx": np.int32,
                 "src_of_cell": np.int32, "link_src": np.int32, "link_dst": np.int32, "tags": np.int32,
                 "zone_rank": np.int32, "rsend_idx": np.int32, "rsend_dst": np.int32, "rsend_peer": np.int32,
-                "rrecv_idx": np.int32, "rsend_off": np.int64, "rrecv_off": np.int64,
+                "rrecv_idx": np.int32, "send_cells": np.int32, "rsend_off": np.int64, "rrecv_off": np.int64,
                 "link_off": np.int64, "zone_offset": np.int64, "zone_nowned": np.int64, "zone_ncells": np.int64}
 
 

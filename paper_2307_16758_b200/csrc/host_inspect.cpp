@@ -122,6 +122,7 @@ int64_t swe_host_get(void* hh, const char* name, void* out, int64_t cap_bytes) {
         if (n == "rrecv_idx") return copy_out(h->Z.rrecv_idx, out, cap_bytes);
         if (n == "rsend_off") return copy_out(h->Z.rsend_off, out, cap_bytes);
         if (n == "rrecv_off") return copy_out(h->Z.rrecv_off, out, cap_bytes);
+        if (n == "send_cells") return copy_out(h->Z.send_cells, out, cap_bytes);
         if (n == "zone_offset" || n == "zone_nowned" || n == "zone_ncells") {
             std::vector<int64_t> v;
             for (const ZoneDesc& zd : h->Z.z)

@@ -541,6 +541,15 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         Z.rsend_off[p + 1] = (int64_t)Z.rsend_idx.size();
         Z.rrecv_off[p + 1] = (int64_t)Z.rrecv_idx.size();
     }
+    // ---- cells on any send list (remote or resident), ascending: the overlap schedule updates them
+    // first; they carry -1 in c2e.w (owned cells otherwise carry 0) ----
+    if (nranks > 1) {
+        Z.send_cells = Z.rsend_idx;
+        Z.send_cells.insert(Z.send_cells.end(), Z.send_idx.begin(), Z.send_idx.end());
+        std::sort(Z.send_cells.begin(), Z.send_cells.end());
+        Z.send_cells.erase(std::unique(Z.send_cells.begin(), Z.send_cells.end()), Z.send_cells.end());
+        for (int32_t c : Z.send_cells) M.c2e[4 * (int64_t)c + 3] = -1;
+    }
     return true;
 }
 

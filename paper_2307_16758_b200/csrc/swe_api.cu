@@ -93,6 +93,8 @@ struct swe_ctx {
     double4** d_peerB = nullptr;
     std::vector<void*> peerA, peerB;   // host copies; [rank] = this context's own buffers
     std::vector<char> peer_ipc;        // 1: opened with cudaIpcOpenMemHandle (closed in free_zones)
+    int* d_send_cells = nullptr;       // distinct cells on a send list (overlap schedule updates them first)
+    int64_t nsendcells = 0;
     // staging for host pointers
     double* d_stage = nullptr;
     size_t stage_elems = 0;
@@ -259,6 +261,8 @@ void free_zones(swe_ctx* c) {
     if (c->d_sendbuf) cudaFree(c->d_sendbuf);
     if (c->d_rsend_idx) cudaFree(c->d_rsend_idx);
     if (c->d_rrecv_idx) cudaFree(c->d_rrecv_idx);
+    if (c->d_send_cells) cudaFree(c->d_send_cells);
+    c->d_send_cells = nullptr; c->nsendcells = 0;
     if (c->d_rsend_dst) cudaFree(c->d_rsend_dst);
     if (c->d_rsend_peer) cudaFree(c->d_rsend_peer);
     if (c->d_peerA) cudaFree(c->d_peerA);
@@ -296,14 +300,29 @@ void run_flux(swe_ctx* c, Store& st, const double4* U, int scheme) {
         else k_edge_flux<K_MUSCL_MS><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
     });
 }
-// mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in
-void run_update(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout, int mode, bool fuse) {
+// mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in;
+// part 0: every owned cell, 1: only the cells on a send list, 2: every owned cell but those
+void run_update(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout, int mode, bool fuse, int part = 0) {
+    if (part == 1) {
+        const int n = (int)c->nsendcells;
+        if (n == 0) return;
+        launch(c, KIND_UPDATE, [&] {
+            const int gr = grid_for(n, c->grid_light);
+            const int* L = c->d_send_cells;
+            if (mode == 0 && !fuse) k_cell_update_list<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else if (mode == 0) k_cell_update_list<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else if (!fuse) k_cell_update_list<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else k_cell_update_list<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+        });
+        return;
+    }
+    const int skip = part == 2 ? 1 : 0;
     launch(c, KIND_UPDATE, [&] {
         const int gr = grid_for(st.nc, c->grid_upd);
-        if (mode == 0 && !fuse) k_cell_update<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
-        else if (mode == 0) k_cell_update<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
-        else if (!fuse) k_cell_update<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
-        else k_cell_update<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S);
+        if (mode == 0 && !fuse) k_cell_update<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
+        else if (mode == 0) k_cell_update<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
+        else if (!fuse) k_cell_update<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
+        else k_cell_update<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
     });
 }
 void run_exchange_state(swe_ctx* c, double4* U, int64_t first, int64_t count, bool do_pack, bool do_unpack) {
@@ -807,6 +826,9 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
         CU(cudaMemcpyAsync(c->d_rsend_dst, c->Z.rsend_dst.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         CU(cudaMemcpyAsync(c->d_rsend_peer, c->Z.rsend_peer.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     }
+    c->nsendcells = (int64_t)c->Z.send_cells.size();
+    CU(cudaMalloc((void**)&c->d_send_cells, (size_t)(c->nsendcells ? c->nsendcells : 1) * sizeof(int)));
+    if (c->nsendcells) CU(cudaMemcpyAsync(c->d_send_cells, c->Z.send_cells.data(), c->nsendcells * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMalloc((void**)&c->d_peerA, (size_t)nranks * sizeof(double4*)));
     CU(cudaMalloc((void**)&c->d_peerB, (size_t)nranks * sizeof(double4*)));
     c->peerA.assign(nranks, nullptr); c->peerB.assign(nranks, nullptr); c->peer_ipc.assign(nranks, 0);
@@ -976,7 +998,7 @@ int swe_dist_begin_step(swe_ctx* c, const double* min_in, double cfl) {
     return SWE_OK;
 }
 
-int swe_dist_stage(swe_ctx* c, int scheme, int stage) {
+static int check_stage(swe_ctx* c, int scheme, int stage) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (scheme < 0 || scheme > 3 || stage < 0 || stage > 1) return fail(SWE_ERR_ARG, "bad stage arguments");
     if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
@@ -984,16 +1006,35 @@ int swe_dist_stage(swe_ctx* c, int scheme, int stage) {
         return fail(SWE_ERR_STATE, "distributed MUSCL / WAF stages need zones with at least 2 ghost layers");
     const bool heun = scheme == K_MUSCL || scheme == K_MUSCL_MS;
     if (!heun && stage != 0) return fail(SWE_ERR_ARG, "Euler schemes have one stage");
+    return SWE_OK;
+}
+
+int swe_dist_flux(swe_ctx* c, int scheme, int stage) {
+    int rc = check_stage(c, scheme, stage); if (rc) return rc;
     Store& st = c->z;
     const double4* Uin = (stage == 0) ? st.A : st.B;
     if (scheme == K_MUSCL) run_grad(c, st, Uin);
     run_flux(c, st, Uin, scheme);
-    if (heun && stage == 0) run_update(c, st, st.A, nullptr, st.B, 0, false);
-    else if (heun) run_update(c, st, st.B, st.A, st.A, 1, true);
-    else run_update(c, st, st.A, nullptr, st.A, 0, true);
-    if (!heun || stage == 1) { c->min_valid = true; c->steps++; }
     CU(cudaGetLastError());
     return SWE_OK;
+}
+
+int swe_dist_update(swe_ctx* c, int scheme, int stage, int part) {
+    int rc = check_stage(c, scheme, stage); if (rc) return rc;
+    if (part < 0 || part > 2) return fail(SWE_ERR_ARG, "part must be 0 (all), 1 (send cells) or 2 (the rest)");
+    const bool heun = scheme == K_MUSCL || scheme == K_MUSCL_MS;
+    Store& st = c->z;
+    if (heun && stage == 0) run_update(c, st, st.A, nullptr, st.B, 0, false, part);
+    else if (heun) run_update(c, st, st.B, st.A, st.A, 1, true, part);
+    else run_update(c, st, st.A, nullptr, st.A, 0, true, part);
+    if ((!heun || stage == 1) && part != 1) { c->min_valid = true; c->steps++; }
+    CU(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_dist_stage(swe_ctx* c, int scheme, int stage) {
+    int rc = swe_dist_flux(c, scheme, stage); if (rc) return rc;
+    return swe_dist_update(c, scheme, stage, 0);
 }
 
 int swe_get_time(swe_ctx* c, double* t_out, double* last_dt_out) {

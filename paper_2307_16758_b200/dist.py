@@ -107,6 +107,21 @@ class TorchComm:
         else:
             self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
 
+    def allreduce_min_async(self, t):
+        """Starts the MIN all-reduce behind the work already on the current stream and returns a
+        handle for wait(): later work on the current stream overlaps with it (nccl; with gloo the
+        host-staged reduction is done at once and None is returned)."""
+        if self.staged_host:
+            self.allreduce_min(t)
+            return None
+        return self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN, async_op=True)
+
+    @staticmethod
+    def wait(work):
+        """Makes the current stream wait for an asynchronous collective (the host does not block)."""
+        if work is not None:
+            work.wait()
+
     def all_to_all(self, recv, send, recv_splits, send_splits):
         if self.staged_host and send.is_cuda:
             r = recv.cpu()
@@ -149,7 +164,8 @@ class DistSolver:
     kernel per exchange) or "staged" (pack -> all-to-all -> unpack).
     """
 
-    def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None):
+    def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None,
+                 schedule="overlap"):
         import torch
         from . import binding as sw
         self.sw, self.torch = sw, torch
@@ -158,6 +174,11 @@ class DistSolver:
         if transport not in ("p2p", "staged"):
             raise ValueError("transport must be 'p2p' or 'staged'")
         self.transport = transport
+        if schedule not in ("plain", "overlap"):
+            raise ValueError("schedule must be 'plain' or 'overlap'")
+        self.schedule = schedule
+        self._bar = self._minwork = None
+        self._primed = False
         if nzones is None:
             nzones = 1
             while nzones < self.world:
@@ -200,6 +221,8 @@ class DistSolver:
 
     def step(self, nsteps, cfl, scheme):
         """nsteps time steps, asynchronous on the current stream (nccl)."""
+        if self.schedule == "overlap":
+            return self._step_overlap(nsteps, cfl, scheme)
         sw = self.sw
         sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
         heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
@@ -218,10 +241,72 @@ class DistSolver:
             elif p2p:
                 self.barrier_stream()                  # everybody has read its ghosts of buffer 0
 
+    # -- overlap schedule (scope row f2; "high overlap") ------------------------------
+    # Every stage updates the cells on the send lists first, exchanges them, starts the barrier
+    # asynchronously and updates the rest of the domain while the collective is in flight; the
+    # all-reduce of dt likewise runs behind the next gradient / flux pass (dt is first needed by
+    # the update; WAF needs it in the flux).  Hazards (buffer b = 0: U, 1: the Heun stage buffer):
+    #   * a rank reads its ghosts of b only after wait(barrier) of the exchange of b;
+    #   * an exchange of b is issued after a wait() on a collective that every rank started after
+    #     its last flux pass over b, so nobody's ghosts are overwritten while still being read.
+    #     Heun: the barrier of the other buffer's exchange is that collective.  Euler schemes have
+    #     one buffer: they start one more barrier right after the flux pass and wait for it before
+    #     the exchange.
+    def _exchange_async(self, buffer):
+        self.exchange(buffer)
+        return self.comm.allreduce_min_async(self.token) if self.transport == "p2p" else None
+
+    def _step_overlap(self, nsteps, cfl, scheme):
+        sw, comm = self.sw, self.comm
+        sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
+        heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
+        waf = sch == sw.SWE_WAF
+        p2p = self.transport == "p2p"
+        for _ in range(int(nsteps)):
+            if not self._primed:                       # first step after set-up / set_state
+                self._bar = self._exchange_async(0)
+                sw.swe_dist_local_min(self.ctx, self.minbuf)
+                self._minwork = comm.allreduce_min_async(self.minbuf)
+                self._primed = True
+            comm.wait(self._bar)                       # ghosts of buffer 0 are current
+            if waf:
+                comm.wait(self._minwork)
+                sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+            sw.swe_dist_flux(self.ctx, sch, 0)
+            if not waf:
+                comm.wait(self._minwork)
+                sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+            if heun:
+                sw.swe_dist_update(self.ctx, sch, 0, 1)            # send cells of U'
+                bar1 = self._exchange_async(1)
+                sw.swe_dist_update(self.ctx, sch, 0, 2)            # the rest, behind the barrier
+                comm.wait(bar1)
+                sw.swe_dist_flux(self.ctx, sch, 1)
+                sw.swe_dist_update(self.ctx, sch, 1, 1)            # send cells of U^{n+1}
+                self._bar = self._exchange_async(0)
+                sw.swe_dist_update(self.ctx, sch, 1, 2)
+            else:
+                done = comm.allreduce_min_async(self.token) if p2p else None   # everybody's flux pass is over
+                sw.swe_dist_update(self.ctx, sch, 0, 1)
+                comm.wait(done)
+                self._bar = self._exchange_async(0)
+                sw.swe_dist_update(self.ctx, sch, 0, 2)
+            sw.swe_dist_local_min(self.ctx, self.minbuf)
+            self._minwork = comm.allreduce_min_async(self.minbuf)
+
+    def _drain(self):
+        """Completes the collectives the overlap schedule left in flight (the ghosts of buffer 0 are
+        then current and minbuf holds the global minimum)."""
+        self.comm.wait(self._bar)
+        self.comm.wait(self._minwork)
+        self._bar = self._minwork = None
+
     def time(self):
         return self.sw.swe_get_time(self.ctx)
 
     def set_state(self, h, hu, hv):
+        self._drain()
+        self._primed = False
         self.comm.host_barrier()
         self.sw.swe_set_state(self.ctx, h, hu, hv)
         self.comm.host_barrier()
@@ -239,6 +324,7 @@ class DistSolver:
         return tuple(o.cpu().numpy() for o in out)
 
     def close(self):
+        self._drain()
         self.comm.host_barrier()                       # nobody still pushes into this rank's buffers
         self.sw.swe_mesh_destroy(self.ctx)
         self.ctx = None

@@ -68,7 +68,9 @@ class _Ranks:
         for r, c in enumerate(self.ctx):
             sw.swe_halo_unpack(c, buffer, self.recvbuf[r])
 
-    def step(self, nsteps, cfl, scheme):
+    def step(self, nsteps, cfl, scheme, overlap=False):
+        if overlap:
+            return self.step_overlap(nsteps, cfl, scheme)
         heun = scheme in ("muscl", "muscl_ms")
         for _ in range(nsteps):
             self.exchange(0)
@@ -83,6 +85,31 @@ class _Ranks:
                 for c in self.ctx:
                     sw.swe_dist_stage(c, scheme, 1)
 
+    def step_overlap(self, nsteps, cfl, scheme):
+        """The phases of DistSolver._step_overlap: send cells first, exchange, then the rest."""
+        heun = scheme in ("muscl", "muscl_ms")
+        self.exchange(0)
+        for _ in range(nsteps):
+            for r, c in enumerate(self.ctx):
+                sw.swe_dist_local_min(c, self.mins[r:r + 1])
+            m = self.mins.min().reshape(1)
+            for c in self.ctx:
+                if scheme == "waf":
+                    sw.swe_dist_begin_step(c, m, cfl)
+                sw.swe_dist_flux(c, scheme, 0)
+                if scheme != "waf":
+                    sw.swe_dist_begin_step(c, m, cfl)
+                sw.swe_dist_update(c, scheme, 0, 1)
+            if heun:
+                self.exchange(1)
+                for c in self.ctx:
+                    sw.swe_dist_update(c, scheme, 0, 2)
+                    sw.swe_dist_flux(c, scheme, 1)
+                    sw.swe_dist_update(c, scheme, 1, 1)
+            self.exchange(0)
+            for c in self.ctx:
+                sw.swe_dist_update(c, scheme, 1 if heun else 0, 2)
+
     def state(self, n):
         out = [np.full(n, np.nan) for _ in range(3)]
         for c in self.ctx:
@@ -95,17 +122,17 @@ class _Ranks:
             sw.swe_mesh_destroy(c)
 
 
-@pytest.mark.parametrize("transport", ["p2p", "staged"])
+@pytest.mark.parametrize("transport,overlap", [("p2p", False), ("staged", False), ("p2p", True)])
 @pytest.mark.parametrize("world,nz,nl", [(2, 2, 2), (4, 4, 2), (2, 8, 3), (3, 8, 2)])
 @pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
-def test_ranks_in_one_process_bit_identical(transport, world, nz, nl, scheme, cfl):
+def test_ranks_in_one_process_bit_identical(transport, overlap, world, nz, nl, scheme, cfl):
     cfg = _river()
     a = sw.create_from_config(cfg)
     R = _Ranks(cfg, world, nz, nl, transport)
     try:
         n = sw.swe_mesh_info(a)["ncell"]
         ta = sw.swe_step(a, 30, cfl, scheme)
-        R.step(30, cfl, scheme)
+        R.step(30, cfl, scheme, overlap)
         ref = sw.swe_get_state(a)
         got = R.state(n)
         for x, y in zip(ref, got):
@@ -154,7 +181,7 @@ def test_one_layer_hllc_and_errors():
         R.close()
 
 
-def _worker(rank, world, port, transport, scheme, cfl, q):
+def _worker(rank, world, port, transport, scheme, cfl, schedule, q):
     sys.path.insert(0, ROOT)
     os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
                       MASTER_PORT=str(port), SWE_DIST_GLOO="1")
@@ -162,8 +189,9 @@ def _worker(rank, world, port, transport, scheme, cfl, q):
         from paper_2307_16758_b200 import dist as d
         d.init_from_env()
         cfg = _river()
-        S = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport)
-        S.step(25, cfl, scheme)
+        S = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport, schedule=schedule)
+        S.step(10, cfl, scheme)
+        S.step(15, cfl, scheme)            # the overlap schedule carries collectives across calls
         t = S.time()
         st = S.get_state()
         S.close()
@@ -181,12 +209,14 @@ def _worker(rank, world, port, transport, scheme, cfl, q):
         q.put((rank, False, traceback.format_exc() + str(e)))
 
 
-@pytest.mark.parametrize("transport,scheme,cfl", [("p2p", "muscl", 0.45), ("staged", "muscl", 0.45), ("p2p", "hllc", 0.9)])
-def test_two_processes_one_gpu_dist_solver(transport, scheme, cfl):
+@pytest.mark.parametrize("transport,scheme,cfl,schedule", [
+    ("p2p", "muscl", 0.45, "overlap"), ("p2p", "muscl", 0.45, "plain"), ("staged", "muscl", 0.45, "overlap"),
+    ("p2p", "hllc", 0.9, "overlap"), ("p2p", "waf", 0.45, "overlap"), ("staged", "hllc", 0.9, "plain")])
+def test_two_processes_one_gpu_dist_solver(transport, scheme, cfl, schedule):
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = 29700 + os.getpid() % 90
-    ps = [ctx.Process(target=_worker, args=(r, 2, port, transport, scheme, cfl, q)) for r in range(2)]
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, transport, scheme, cfl, schedule, q)) for r in range(2)]
     for p in ps:
         p.start()
     try:

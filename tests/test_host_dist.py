@@ -29,7 +29,7 @@ def _build(cfg, nz, nl, world, rank):
     h = sw.swe_host_mesh_build(cfg["x"], cfg["y"], cfg["zb"], cfg["tri"], cfg["bedge"], cfg["btag"])
     sw.swe_host_zones_build_dist(h, nz, nl, None, world, rank, swdist.zone_blocks(nz, world))
     names = ("zone_rank", "rsend_idx", "rsend_dst", "rsend_peer", "rrecv_idx", "rsend_off", "rrecv_off",
-             "z:cell_user", "z:c2c", "zone_offset", "zone_ncells", "zone_nowned", "send_idx", "recv_idx")
+             "z:cell_user", "z:c2c", "z:c2e", "send_cells", "zone_offset", "zone_ncells", "zone_nowned", "send_idx", "recv_idx")
     out = {n: sw.swe_host_get(h, n) for n in names}
     sw.swe_host_mesh_free(h)
     return out
@@ -68,6 +68,12 @@ def test_ranks_agree_on_the_halo_lists(world, nz, nl):
         lay = R[a]["z:c2c"].reshape(-1, 4)[:, 3]
         assert np.all(lay[R[a]["rsend_idx"]] == 0) and np.all(lay[R[a]["rrecv_idx"]] > 0)
         assert np.all(lay[R[a]["send_idx"]] == 0) and np.all(lay[R[a]["recv_idx"]] > 0)
+        # the overlap schedule's "send cells": every cell on a send list once, marked -1 in c2e.w
+        sc = R[a]["send_cells"]
+        assert np.array_equal(sc, np.unique(np.concatenate([R[a]["rsend_idx"], R[a]["send_idx"]])))
+        mark = R[a]["z:c2e"].reshape(-1, 4)[:, 3]
+        assert np.array_equal(np.flatnonzero(mark == -1), sc)
+        assert np.array_equal(mark > 0, lay > 0) and np.all(mark[(lay == 0)] <= 0)
         # every ghost slot is fed exactly once: by a resident zone or by a peer
         fed = np.concatenate([R[a]["recv_idx"], R[a]["rrecv_idx"]])
         assert np.array_equal(np.sort(fed), np.flatnonzero(lay > 0))
