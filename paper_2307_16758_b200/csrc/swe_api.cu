@@ -112,8 +112,8 @@ struct swe_ctx {
 
 namespace {
 
-int grid_for(int64_t n, int cap) {
-    int64_t b = (n + 255) / 256;
+int grid_for(int64_t n, int cap, int threads = 256) {
+    int64_t b = (n + threads - 1) / threads;
     if (b < 1) b = 1;
     return (int)(b < cap ? b : cap);
 }
@@ -288,16 +288,16 @@ void run_dt_reduce(swe_ctx* c, Store& st, const double4* U) {
 }
 void run_grad(swe_ctx* c, Store& st, const double4* U) {
     launch(c, KIND_GRAD, [&] {
-        k_grad_limit<<<grid_for(st.nc, c->grid_grad), 256, 0, c->stream>>>(st.dm, U, st.grad, c->P);
+        k_grad_limit<<<grid_for(st.nc, c->grid_grad, SWE_GRAD_THREADS), SWE_GRAD_THREADS, 0, c->stream>>>(st.dm, U, st.grad, c->P);
     });
 }
 void run_flux(swe_ctx* c, Store& st, const double4* U, int scheme) {
     launch(c, KIND_FLUX, [&] {
-        const int gr = grid_for(st.ne, c->grid_flux[scheme]);
-        if (scheme == K_HLLC) k_edge_flux<K_HLLC><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else if (scheme == K_MUSCL) k_edge_flux<K_MUSCL><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else if (scheme == K_WAF) k_edge_flux<K_WAF><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else k_edge_flux<K_MUSCL_MS><<<gr, 256, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        const int gr = grid_for(st.ne, c->grid_flux[scheme], SWE_FLUX_THREADS);
+        if (scheme == K_HLLC) k_edge_flux<K_HLLC><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else if (scheme == K_MUSCL) k_edge_flux<K_MUSCL><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else if (scheme == K_WAF) k_edge_flux<K_WAF><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        else k_edge_flux<K_MUSCL_MS><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
     });
 }
 // mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in;
@@ -416,17 +416,17 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) c->num_sm = prop.multiProcessorCount;
     // persistent grids: (resident blocks per SM) x (SM count), from the occupancy calculator
-    auto occ = [&](const void* k, int fallback) {
+    auto occ = [&](const void* k, int fallback, int threads = 256) {
         int nbk = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k, 256, 0) != cudaSuccess || nbk < 1) { cudaGetLastError(); nbk = fallback; }
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k, threads, 0) != cudaSuccess || nbk < 1) { cudaGetLastError(); nbk = fallback; }
         return nbk * c->num_sm;
     };
     c->grid_light = 8 * c->num_sm;
-    c->grid_grad = occ((const void*)k_grad_limit, 4);
-    c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC>, 4);
-    c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2);
-    c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2);
-    c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS>, 2);
+    c->grid_grad = occ((const void*)k_grad_limit, 4, SWE_GRAD_THREADS);
+    c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC>, 4, SWE_FLUX_THREADS);
+    c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2, SWE_FLUX_THREADS);
+    c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2, SWE_FLUX_THREADS);
+    c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS>, 2, SWE_FLUX_THREADS);
     c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
