@@ -158,4 +158,25 @@ def simple_wave_case(nx, ny=None, lx=100.0, ly=None, jitter=0.0, seed=0, h0=1.0,
     return cfg
 
 
+def channel_flow_case(nx=100, ny=5, lx=100.0, ly=5.0, jitter=0.1, seed=4, discharge=10.0, level=2.0,
+                      manning=0.0, h_init=None, u_init=0.0):
+    """Straight flat channel with the two open boundaries of configs[3]: imposed discharge Q on the
+    upstream side x = 0 (tag 1), fixed water level on the downstream side x = lx (tag 2), walls on
+    the long sides.  Initial state: depth h_init (default: the level) and velocity u_init along x,
+    uniform.  Used to pin the oracle's open boundaries (uniform flow, backwater curve)."""
+    x, y, tri = grid_mesh(nx, ny, lx, ly, jitter, seed)
+    j = np.arange(ny)
+    west = np.stack([j * (nx + 1), (j + 1) * (nx + 1)], axis=1)
+    east = west + nx
+    bedge = np.concatenate([west, east], axis=0)
+    btag = np.concatenate([np.full(ny, 1), np.full(ny, 2)]).astype(np.int32)
+    nt = tri.shape[0]
+    h0 = float(level if h_init is None else h_init)
+    cfg = _base("channel_flow", x, y, np.zeros_like(x), tri, np.full(nt, h0), [("hllc", 0.9, 0)],
+                manning=np.full(nt, float(manning)) if manning else None, bedge=bedge, btag=btag,
+                bc={1: ("inflow", float(discharge)), 2: ("level", float(level))})
+    cfg["hu"] = np.full(nt, h0 * float(u_init))
+    return cfg
+
+
 CONFIG_BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3}

@@ -1,0 +1,93 @@
+"""Pins for the oracle's open boundaries ("incoming flow Q", and the fixed water level
+the paper uses at PAPER.md:518, 548 without defining it; readings R10, R11) against what
+the mathematics fixes, on a straight flat channel with inflow Q upstream and a level downstream:
+
+ * uniform subcritical flow h = level, u = Q/(W h) is an exact steady solution of the equations
+   and of both boundary formulas: it must be preserved to round-off by every scheme (a wrong sign,
+   magnitude or per-width distribution of Q, or a wrong ghost depth, breaks it at once);
+ * with Manning friction the steady state is the gradually-varied-flow (backwater) profile
+       dh/dx = -S_f / (1 - Fr^2),  S_f = n^2 q^2 / h^(10/3),  Fr^2 = q^2 / (g h^3),  h(L) = level,
+   a textbook ODE integrated here with scipy, independently of the oracle: the oracle started from
+   still water must relax to it (first-order accurate: the error halves with the mesh size), with
+   the discharge per unit width equal to Q / W along the whole channel.
+"""
+import numpy as np
+import pytest
+from scipy.integrate import solve_ivp
+
+import swe_inputs as si
+from oracle import pyoracle as po
+
+G = 9.81
+
+
+@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_uniform_flow_is_an_exact_steady_state(scheme, cfl, oracle_threads):
+    Q, level, W = 10.0, 2.0, 5.0
+    u0 = Q / (W * level)                       # Fr = 0.23: subcritical
+    cfg = si.channel_flow_case(discharge=Q, level=level, u_init=u0)
+    o = po.Oracle.from_config(cfg)
+    o.step(200, cfl, scheme)
+    h, hu, hv = o.get_state()
+    assert np.abs(h - level).max() < 1e-13
+    assert np.abs(hu - level * u0).max() < 1e-13
+    assert np.abs(hv).max() < 1e-13
+
+
+def test_wrong_discharge_does_not_keep_the_uniform_flow(oracle_threads):
+    # the same state with half the discharge imposed is NOT steady: the pin above can fail
+    cfg = si.channel_flow_case(discharge=5.0, level=2.0, u_init=1.0)
+    o = po.Oracle.from_config(cfg)
+    o.step(50, 0.9, "hllc")
+    h, hu, hv = o.get_state()
+    assert np.abs(hu - 2.0).max() > 0.1
+
+
+def _backwater(x, q, n, level, length):
+    f = lambda s, h: -(n * n * q * q / h ** (10.0 / 3.0)) / (1.0 - q * q / (G * h ** 3))
+    sol = solve_ivp(f, [length, 0.0], [level], dense_output=True, rtol=1e-10, atol=1e-12)
+    return sol.sol(x)[0]
+
+
+def _relax(scheme, cfl, nx, steps):
+    n, Q, level, lx, ly = 0.03, 20.0, 1.0, 200.0, 10.0
+    cfg = si.channel_flow_case(nx=nx, ny=nx // 20, lx=lx, ly=ly, discharge=Q, level=level, manning=n)
+    o = po.Oracle.from_config(cfg)
+    o.step(steps, cfl, scheme)
+    h, hu, hv = o.get_state()
+    cx = cfg["x"][cfg["tri"]].mean(axis=1)
+    he = _backwater(cx, Q / ly, n, level, lx)
+    return h, hu, hv, cx, he, Q / ly
+
+
+def test_backwater_curve_hllc_first_order(oracle_threads):
+    errs = []
+    for nx, steps in ((100, 8000), (200, 16000)):
+        h, hu, hv, cx, he, q = _relax("hllc", 0.9, nx, steps)
+        errs.append(np.abs(h - he).mean() / he.mean())
+        assert np.abs(hu - q).max() < 0.01 * q            # discharge per unit width = Q / W everywhere
+        assert np.abs(hv).max() < 0.01 * q
+        # inlet depth of the M-type curve (1.447 m for these numbers) and the imposed outlet level
+        assert abs(h[cx < 4.0].mean() - he[cx < 4.0].mean()) < 5e-3
+        assert abs(h[cx > 196.0].mean() - he[cx > 196.0].mean()) < 5e-3
+    assert errs[0] < 1.0e-3 and errs[1] < 0.6 * errs[0], errs
+    assert 1.40 < h[cx < 4.0].mean() < 1.46           # the M-type curve rises 0.44 m above the level
+
+
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_backwater_curve_second_order_schemes(scheme, cfl, oracle_threads):
+    h, hu, hv, cx, he, q = _relax(scheme, cfl, 100, 12000)
+    assert np.abs(h - he).mean() / he.mean() < 1.0e-3
+    assert np.abs(h - he).max() < 0.01
+    assert np.abs(hu - q).max() < 0.025 * q
+
+
+def test_backwater_reference_is_the_textbook_curve():
+    # the ODE solution used above against its own closed-form check: x(h) by quadrature of
+    # dx/dh = -(1 - Fr^2)/S_f from the outlet depth (independent of solve_ivp)
+    q, n, level, L = 2.0, 0.03, 1.0, 200.0
+    hs = np.linspace(level, 1.4, 4001)
+    dxdh = -(1.0 - q * q / (G * hs ** 3)) / (n * n * q * q / hs ** (10.0 / 3.0))
+    x_of_h = L + np.concatenate([[0.0], np.cumsum(0.5 * (dxdh[1:] + dxdh[:-1]) * np.diff(hs))])
+    for k in (500, 2000, 4000):
+        assert abs(_backwater(np.array([x_of_h[k]]), q, n, level, L)[0] - hs[k]) < 1e-6
