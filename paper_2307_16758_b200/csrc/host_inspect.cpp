@@ -44,6 +44,8 @@ int64_t mesh_get(const MeshArrays& M, const std::string& n, void* out, int64_t c
     if (n == "btag") return copy_out(M.btag, out, cap);
     if (n == "dupw") return copy_out(M.dupw, out, cap);
     if (n == "edlr") return copy_out(M.edlr, out, cap);
+    if (n == "eside") return copy_out(M.eside, out, cap);
+    if (n == "ernorm") return copy_out(M.ernorm, out, cap);
     return -2;
 }
 }  // namespace

@@ -282,6 +282,19 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         const double ux = H.cx[R] - H.cx[L], uy = H.cy[R] - H.cy[L];
         M.edlr[d] = std::sqrt(ux * ux + uy * uy);
     }
+    M.ernorm.assign(2 * (size_t)ne, 0.0);
+    for (int64_t d = 0; d < ne; ++d) {
+        M.ernorm[2 * d] = std::sqrt(M.erl[2 * d] * M.erl[2 * d] + M.erl[2 * d + 1] * M.erl[2 * d + 1]);
+        M.ernorm[2 * d + 1] = std::sqrt(M.err[2 * d] * M.err[2 * d] + M.err[2 * d + 1] * M.err[2 * d + 1]);
+    }
+    // local side index of every edge in its two cells (the multislope slopes are stored per side)
+    M.eside.assign(ne, 0);
+    for (int64_t i = 0; i < nt; ++i)
+        for (int k = 0; k < 3; ++k) {
+            const int32_t ce = M.c2e[4 * i + k];
+            if (ce >= 0) M.eside[ce] |= (uint8_t)k;
+            else M.eside[~ce] |= (uint8_t)(k << 2);
+        }
 
     // distinct tags and their widths (sum of edge lengths, reading R10)
     for (int64_t b = 0; b < nbe; ++b) {
@@ -456,6 +469,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     if (M.ne > (int64_t)INT32_MAX / 2) { err = "zoned mesh too large"; return false; }
     M.elr.resize(2 * M.ne); M.en.resize(2 * M.ne); M.elen.resize(M.ne); M.edx.resize(M.ne);
     M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne); M.edlr.resize(M.ne);
+    M.eside.resize(M.ne); M.ernorm.resize(2 * M.ne);
     M.dupw.assign(4 * (size_t)ncz, 0.0);
     M.btag.assign(M.ne - M.ne_int, -1);
     std::vector<int32_t> eloc(G.ne, -1);
@@ -469,7 +483,8 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             M.elr[2 * d] = (int32_t)(o + loc[L]);
             M.elr[2 * d + 1] = R >= 0 ? (int32_t)(o + loc[R]) : -1;
             M.en[2 * d] = G.en[2 * (int64_t)e]; M.en[2 * d + 1] = G.en[2 * (int64_t)e + 1];
-            M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e]; M.edlr[d] = G.edlr[e];
+            M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e]; M.edlr[d] = G.edlr[e]; M.eside[d] = G.eside[e];
+            M.ernorm[2 * d] = G.ernorm[2 * (int64_t)e]; M.ernorm[2 * d + 1] = G.ernorm[2 * (int64_t)e + 1];
             M.erl[2 * d] = G.erl[2 * (int64_t)e]; M.erl[2 * d + 1] = G.erl[2 * (int64_t)e + 1];
             M.err[2 * d] = G.err[2 * (int64_t)e]; M.err[2 * d + 1] = G.err[2 * (int64_t)e + 1];
             eloc[e] = (int32_t)d;

@@ -30,6 +30,8 @@ struct MeshArrays {
     std::vector<double> elen, edx;           // length, WAF Delta-x
     std::vector<double> erl, err;            // 2*ne each: r_{L,e}, r_{R,e}
     std::vector<double> edlr;                // |x_R - x_L| between the centroids (0 on the boundary)
+    std::vector<double> ernorm;              // 2*ne: |r_{L,e}|, |r_{R,e}| (multislope MUSCL face distances)
+    std::vector<uint8_t> eside;              // ne: local side of the edge in its L cell | (in its R cell) << 2
     std::vector<int32_t> btag;               // ne-ne_int: user tag of the boundary edge (-1 = none)
 };
 

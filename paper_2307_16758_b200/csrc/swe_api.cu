@@ -105,6 +105,7 @@ struct swe_ctx {
     int64_t prof_n[NKIND] = {0};
     // grid sizes (persistent grid-stride kernels: a multiple of the SM count)
     int grid_light = 148 * 8;
+    int grid_ms = 148 * 5;
     int grid_grad = 148 * 4, grid_flux[4] = {148 * 4, 148 * 2, 148 * 2, 148 * 2}, grid_upd = 148 * 8;
 
     Store& active() { return has_zones ? z : g; }
@@ -187,10 +188,13 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.upload(&erl, M.erl.data(), (size_t)M.ne, s));
     CU(st.upload(&err, M.err.data(), (size_t)M.ne, s));
     d.elr = elr; d.en = en; d.elen = elen; d.edx = edx; d.erl = erl; d.err = err;
-    double4* dupw; double* edlr;
+    double4* dupw; double* edlr; uint8_t* eside;
     CU(st.upload(&dupw, M.dupw.data(), (size_t)M.nc, s));
     CU(st.upload(&edlr, M.edlr.data(), (size_t)M.ne, s));
-    d.dupw = dupw; d.edlr = edlr;
+    CU(st.upload(&eside, M.eside.data(), (size_t)M.ne, s));
+    double2* ernorm;
+    CU(st.upload(&ernorm, M.ernorm.data(), (size_t)M.ne, s));
+    d.dupw = dupw; d.edlr = edlr; d.eside = eside; d.ernorm = ernorm;
     CU(st.upload(&st.d_cell_user, M.cell_user.data(), (size_t)M.nc, s));
     CU(st.alloc(&st.d_bkind, (size_t)st.nbe));
     CU(st.alloc(&st.d_bval, (size_t)st.nbe));
@@ -199,13 +203,13 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     d.layer = nullptr;
     CU(st.alloc(&st.A, (size_t)M.nc));
     CU(st.alloc(&st.B, (size_t)M.nc));
-    CU(st.alloc(&st.grad, 2 * (size_t)M.nc));
+    CU(st.alloc(&st.grad, 3 * (size_t)M.nc));      // 2 per cell (limited gradients) or 3 (multislope side records)
     CU(st.alloc(&st.F.f1, (size_t)M.ne));
     CU(st.alloc(&st.F.fxl, (size_t)M.ne));
     CU(st.alloc(&st.F.fyl, (size_t)M.ne));
     CU(st.alloc(&st.F.fxr, (size_t)M.ne));
     CU(st.alloc(&st.F.fyr, (size_t)M.ne));
-    CU(cudaMemsetAsync(st.grad, 0, 2 * (size_t)M.nc * sizeof(double4), s));
+    CU(cudaMemsetAsync(st.grad, 0, 3 * (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.B, 0, (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.d_nman, 0, (size_t)(M.nc ? M.nc : 1) * sizeof(double), s));
     return SWE_OK;
@@ -286,7 +290,16 @@ void run_dt_reduce(swe_ctx* c, Store& st, const double4* U) {
         k_dt_reduce<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.dm, U, c->P, c->d_S);
     });
 }
-void run_grad(swe_ctx* c, Store& st, const double4* U) {
+// cell pass ahead of the flux: limited least-squares gradients (MUSCL) or the multislope side
+// records (MUSCL_MS); HLLC and WAF have none
+void run_grad(swe_ctx* c, Store& st, const double4* U, int scheme = K_MUSCL) {
+    if (scheme == K_MUSCL_MS) {
+        launch(c, KIND_GRAD, [&] {
+            k_ms_slopes<<<grid_for(st.nc, c->grid_ms, 128), 128, 0, c->stream>>>(st.dm, U, st.grad, c->P);
+        });
+        return;
+    }
+    if (scheme != K_MUSCL) return;
     launch(c, KIND_GRAD, [&] {
         k_grad_limit<<<grid_for(st.nc, c->grid_grad, SWE_GRAD_THREADS), SWE_GRAD_THREADS, 0, c->stream>>>(st.dm, U, st.grad, c->P);
     });
@@ -355,10 +368,8 @@ void run_exchange_grad(swe_ctx* c) {
 // one Euler stage on the active store: [exchange] -> [grad (-> exchange grad)] -> flux -> update
 void run_stage(swe_ctx* c, Store& st, double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
     if (c->has_zones) run_exchange_state(c, Uin, 0, c->nsend, true, true);
-    if (scheme == K_MUSCL) {
-        run_grad(c, st, Uin);
-        if (c->has_zones && c->Z.nlayers == 1) run_exchange_grad(c);
-    }
+    run_grad(c, st, Uin, scheme);
+    if (scheme == K_MUSCL && c->has_zones && c->Z.nlayers == 1) run_exchange_grad(c);
     run_flux(c, st, Uin, scheme);
     run_update(c, st, Uin, U0, Uout, mode, fuse);
 }
@@ -428,6 +439,7 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2, SWE_FLUX_THREADS);
     c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS>, 2, SWE_FLUX_THREADS);
     c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
+    c->grid_ms = occ((const void*)k_ms_slopes, 5, 128);
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
         cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
@@ -644,7 +656,7 @@ int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out)
     Store& st = c->active();
     const bool prof = c->profile; c->profile = false;
     // make the inputs of the timed kernel valid
-    if (scheme == K_MUSCL && which >= 2) run_grad(c, st, st.A);
+    if (which >= 2) run_grad(c, st, st.A, scheme);
     if (which >= 3 && which <= 4) run_flux(c, st, st.A, scheme);
     cudaEvent_t a, b;
     CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
@@ -652,7 +664,7 @@ int swe_kernel_timed(swe_ctx* c, int which, int scheme, int reps, float* ms_out)
     for (int r = 0; r < reps; ++r) {
         switch (which) {
             case 0: run_dt_reduce(c, st, st.A); break;
-            case 1: run_grad(c, st, st.A); break;
+            case 1: run_grad(c, st, st.A, scheme == K_MUSCL_MS ? K_MUSCL_MS : K_MUSCL); break;
             case 2: run_flux(c, st, st.A, scheme); break;
             case 3: run_update(c, st, st.A, nullptr, st.B, 0, false); break;
             case 4: run_update(c, st, st.B, st.A, st.B, 1, false); break;
@@ -730,7 +742,7 @@ int swe_side_fluxes(swe_ctx* c, double dt, int scheme, double* out) {
     if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
     double* d; int rc = out_to_user(c, out, 9 * (size_t)c->g.nc, &d); if (rc) return rc;
     k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);
-    if (scheme == K_MUSCL) run_grad(c, c->g, c->g.A);
+    run_grad(c, c->g, c->g.A, scheme);
     run_flux(c, c->g, c->g.A, scheme);
     k_side_flux_to_user<<<grid_for(c->g.nc, c->grid_light), 256, 0, c->stream>>>(c->g.dm, c->g.F, c->g.d_cell_user, d);
     CU(cudaGetLastError());
@@ -743,7 +755,7 @@ int swe_euler_stage(swe_ctx* c, double dt, int scheme, double* h1, double* hu1, 
     if (c->has_zones) return fail(SWE_ERR_STATE, "single-pass inspection calls act on the un-zoned mesh");
     const int64_t nt = c->g.nc;
     k_set_dt<<<1, 1, 0, c->stream>>>(c->d_S, dt);
-    if (scheme == K_MUSCL) run_grad(c, c->g, c->g.A);
+    run_grad(c, c->g, c->g.A, scheme);
     run_flux(c, c->g, c->g.A, scheme);
     run_update(c, c->g, c->g.A, nullptr, c->g.B, 0, false);
     const bool dev = is_device_ptr(h1) && is_device_ptr(hu1) && is_device_ptr(hv1);
@@ -1013,7 +1025,7 @@ int swe_dist_flux(swe_ctx* c, int scheme, int stage) {
     int rc = check_stage(c, scheme, stage); if (rc) return rc;
     Store& st = c->z;
     const double4* Uin = (stage == 0) ? st.A : st.B;
-    if (scheme == K_MUSCL) run_grad(c, st, Uin);
+    run_grad(c, st, Uin, scheme);
     run_flux(c, st, Uin, scheme);
     CU(cudaGetLastError());
     return SWE_OK;
