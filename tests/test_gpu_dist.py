@@ -229,3 +229,30 @@ def test_two_processes_one_gpu_dist_solver(transport, scheme, cfl, schedule):
                 p.kill()
     assert all(r[2] == "" for r in res), [r[2] for r in res]
     assert res[0][1] is True
+
+
+@pytest.mark.parametrize("extra", [[], ["--transport", "staged", "--schedule", "plain", "--scheme", "hllc", "--layers", "1"]])
+def test_bench_line_of_the_distributed_arm(extra):
+    """bench.py at N = 2 (two ranks on this GPU, gloo): the contract line of the strong-scaling arm."""
+    import json
+    import subprocess
+    env = dict(os.environ, SWE_DIST_GLOO="1")
+    for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"):
+        env.pop(k, None)
+    port = 29800 + os.getpid() % 90
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "5",
+           "--warmup", "3", "--workload", "c3t", "--e2e-steps", "2"] + extra
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=ROOT, env=env)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 only
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["steps"] == 5 and d["unit"] == "cell-updates/s"
+    assert d["value"] > 0 and abs(d["value"] - d["config"]["cells"] * 5 / (d["ms_per_step"] * 5e-3)) < 1e-6 * d["value"]
+    assert d["config"]["zones"] == 2 and "ranks" in d["config"]["parallelism"] and d["config"]["halo_bytes_per_step"] > 0
+    launches_per_step_per_rank = d["gpu_launches"] / (5 * 2)
+    assert 4 <= launches_per_step_per_rank <= 14
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["achieved"] > 0 and r["peak"] > 0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0 and d["cpu_baseline"] is None
