@@ -192,16 +192,31 @@ class DistSolver:
         dev = torch.device("cuda", torch.cuda.current_device())
         self.minbuf = torch.zeros(1, dtype=torch.float64, device=dev)
         self.token = torch.zeros(1, dtype=torch.float64, device=dev)
-        if transport == "staged":
+        if self.transport == "p2p":
+            # map every peer's state buffers (CUDA IPC); if any rank cannot (no peer access between
+            # two GPUs, IPC not permitted), ALL ranks take the staged transport -- said on stderr
+            handles = self.comm.all_gather_bytes(sw.swe_peer_export(self.ctx))
+            ok, why = 1.0, ""
+            for p in range(self.world):
+                if p != self.rank:
+                    try:
+                        sw.swe_peer_import(self.ctx, p, handles[p])
+                    except sw.SweError as e:
+                        ok, why = 0.0, str(e)
+                        break
+            flag = torch.tensor([ok], dtype=torch.float64, device=dev)
+            self.comm.allreduce_min(flag)
+            if float(flag.item()) < 1.0:
+                import sys
+                if why or self.rank == 0:
+                    sys.stderr.write("[swe dist] rank %d: peer-memory transport unavailable (%s); every rank uses "
+                                     "the staged transport\n" % (self.rank, why or "another rank failed"))
+                self.transport = "staged"
+        if self.transport == "staged":
             self.sendbuf = torch.zeros(max(1, 3 * int(self.send_cells.sum())), dtype=torch.float64, device=dev)
             self.recvbuf = torch.zeros(max(1, 3 * int(self.recv_cells.sum())), dtype=torch.float64, device=dev)
             self.ssplit = [3 * int(v) for v in self.send_cells]
             self.rsplit = [3 * int(v) for v in self.recv_cells]
-        else:
-            handles = self.comm.all_gather_bytes(sw.swe_peer_export(self.ctx))
-            for p in range(self.world):
-                if p != self.rank:
-                    sw.swe_peer_import(self.ctx, p, handles[p])
         self.comm.host_barrier()
 
     # -- one exchange of the ghosts of state buffer `buffer` (0 = U, 1 = the Heun stage buffer) --
