@@ -195,10 +195,15 @@ class DistSolver:
         if self.transport == "p2p":
             # map every peer's state buffers (CUDA IPC); if any rank cannot (no peer access between
             # two GPUs, IPC not permitted), ALL ranks take the staged transport -- said on stderr
-            handles = self.comm.all_gather_bytes(sw.swe_peer_export(self.ctx))
             ok, why = 1.0, ""
+            try:
+                mine = sw.swe_peer_export(self.ctx)
+            except sw.SweError as e:
+                import numpy as np
+                mine, ok, why = np.zeros(128, np.uint8), 0.0, str(e)
+            handles = self.comm.all_gather_bytes(mine)
             for p in range(self.world):
-                if p != self.rank:
+                if ok and p != self.rank:
                     try:
                         sw.swe_peer_import(self.ctx, p, handles[p])
                     except sw.SweError as e:
