@@ -93,6 +93,12 @@ int swe_set_time(swe_ctx* ctx, double t);
  * few ghost layers for the scheme: WAF and MUSCL_MS need 2), SWE_ERR_CUDA. */
 int swe_step(swe_ctx* ctx, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out);
 
+/* swe_step replays one captured CUDA graph per time step when nsteps >= 2 (the step is a fixed
+ * sequence of 3-11 kernels whose only varying input, dt, lives in device memory; on meshes below
+ * ~1 M cells the step is launch-bound).  on = 0 launches the kernels one by one (default: on).  The
+ * results are identical either way. */
+int swe_set_graphs(swe_ctx* ctx, int on);
+
 /* Zone decomposition resident on this GPU.
  *   nzones : number of zones; zone_of_cell (nt, user order, values in [0,nzones)) or NULL =
  *            recursive coordinate bisection (nzones must then be a power of two)

@@ -37,6 +37,7 @@ SIGNATURES = {
     "swe_get_state": (C.c_int, [_vp, _vp, _vp, _vp]),
     "swe_set_time": (C.c_int, [_vp, C.c_double]),
     "swe_step": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, _dp, _dp]),
+    "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
     "swe_zones_create": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_unpack_ghosts": (C.c_int, [_vp, C.c_int]),
@@ -197,6 +198,10 @@ def swe_step(ctx, nsteps, cfl, scheme, sync=True):
     t, dt = C.c_double(), C.c_double()
     _check(lib().swe_step(ctx, int(nsteps), float(cfl), _scheme(scheme), C.byref(t), C.byref(dt)))
     return t.value, dt.value
+
+
+def swe_set_graphs(ctx, on):
+    _check(lib().swe_set_graphs(ctx, 1 if on else 0))
 
 
 def swe_zones_create(ctx, nzones, nlayers, zone_of_cell=None):

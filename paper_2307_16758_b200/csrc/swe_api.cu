@@ -103,6 +103,13 @@ struct swe_ctx {
     std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> prof_events;
     double prof_ms[NKIND] = {0};
     int64_t prof_n[NKIND] = {0};
+    // one time step captured as a CUDA graph and replayed (launch-bound on small meshes): valid for
+    // one (scheme, cfl, store, parameter set); captured on a side stream, launched on `stream`
+    bool use_graphs = true;
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t step_exec = nullptr;
+    int graph_scheme = -1; double graph_cfl = 0.0; bool graph_zoned = false;
+    int64_t graph_launches = 0, graph_halo = 0;
     // grid sizes (persistent grid-stride kernels: a multiple of the SM count)
     int grid_light = 148 * 8;
     int grid_ms = 148 * 5;
@@ -256,7 +263,13 @@ __global__ void k_scatter_owned(double4* __restrict__ dst, const double4* __rest
 }
 __global__ void k_reset_min(StepScalars* S) { S->min_bits = 0x7ff0000000000000ULL; }
 
+void drop_graph(swe_ctx* c) {
+    if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
+    c->step_exec = nullptr; c->graph_scheme = -1;
+}
+
 void free_zones(swe_ctx* c) {
+    drop_graph(c);
     c->z.release();
     c->z = Store();
     if (c->d_send_idx) cudaFree(c->d_send_idx);
@@ -472,6 +485,7 @@ int swe_mesh_destroy(swe_ctx* c) {
     cudaStreamSynchronize(c->stream);
     for (auto& pe : c->prof_events) { cudaEventDestroy(pe.second.first); cudaEventDestroy(pe.second.second); }
     free_zones(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     c->g.release();
     if (c->d_S) cudaFree(c->d_S);
     if (c->d_flag) cudaFree(c->d_flag);
@@ -494,6 +508,7 @@ int swe_set_params(swe_ctx* c, double g, double h_dry, double h_thin, double bet
     if (!(g > 0.0) || !(h_dry >= 0.0) || !(h_thin >= 0.0) || beta != beta) return fail(SWE_ERR_ARG, "bad parameter value");
     c->P.g = g; c->P.h_dry = h_dry; c->P.h_thin = h_thin; c->beta = beta;
     c->P.kappa = beta / 2.0; c->P.inv_g = 1.0 / g; c->P.limited = beta > 0.0 ? 1 : 0;
+    drop_graph(c);                                   // the parameters are kernel arguments
     c->min_valid = false;
     k_reset_min<<<1, 1, 0, c->stream>>>(c->d_S);
     return SWE_OK;
@@ -609,8 +624,7 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
     if (c->has_zones && (scheme == K_WAF || scheme == K_MUSCL_MS) && c->Z.nlayers < 2)
         return fail(SWE_ERR_STATE, "WAF and the multislope MUSCL need zones with at least 2 ghost layers");
     Store& st = c->active();
-    for (int s = 0; s < nsteps; ++s) {
-        if (!c->min_valid) run_dt_reduce(c, st, st.A);                      // a9
+    auto enqueue_step = [&] {
         launch(c, KIND_MISC, [&] { k_dt_finalize<<<1, 1, 0, c->stream>>>(c->d_S, cfl, 1); });
         if (scheme == K_MUSCL || scheme == K_MUSCL_MS) {                    // Heun RK2 (A.11)
             run_stage(c, st, st.A, nullptr, st.B, scheme, 0, false);
@@ -618,7 +632,42 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
         } else {
             run_stage(c, st, st.A, nullptr, st.A, scheme, 0, true);
         }
+    };
+    int s0 = 0;
+    if (nsteps > 0 && !c->min_valid) {                                       // a9, first step after a state change
+        run_dt_reduce(c, st, st.A);
         c->min_valid = true;
+    }
+    if (c->use_graphs && !c->profile && nsteps >= 2) {
+        // capture one step (same kernels, same order, same arguments) and replay it
+        if (!c->step_exec || c->graph_scheme != scheme || c->graph_cfl != cfl || c->graph_zoned != c->has_zones) {
+            drop_graph(c);
+            if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+            const int64_t l0 = c->launches, h0 = c->halo_bytes;
+            cudaStream_t user = c->stream;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                c->stream = c->cap_stream;
+                enqueue_step();
+                c->stream = user;
+                e = cudaStreamEndCapture(c->cap_stream, &graph);
+            }
+            c->graph_launches = c->launches - l0; c->graph_halo = c->halo_bytes - h0;
+            c->launches = l0; c->halo_bytes = h0;
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&c->step_exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { c->step_exec = nullptr; return fail(SWE_ERR_CUDA, std::string("step graph: ") + cudaGetErrorString(e)); }
+            c->graph_scheme = scheme; c->graph_cfl = cfl; c->graph_zoned = c->has_zones;
+        }
+        for (; s0 < nsteps; ++s0) {
+            CU(cudaGraphLaunch(c->step_exec, c->stream));
+            c->launches += c->graph_launches; c->halo_bytes += c->graph_halo;
+            c->steps++;
+        }
+    }
+    for (int s = s0; s < nsteps; ++s) {
+        enqueue_step();
         c->steps++;
     }
     CU(cudaGetLastError());
@@ -630,6 +679,13 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
         if (t_out) *t_out = hs.t;
         if (last_dt_out) *last_dt_out = hs.last_dt;
     }
+    return SWE_OK;
+}
+
+int swe_set_graphs(swe_ctx* c, int on) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    c->use_graphs = on != 0;
+    if (!on) drop_graph(c);
     return SWE_OK;
 }
 

@@ -248,3 +248,34 @@ def test_mesh_errors_through_the_gpu_entry_point():
     with pytest.raises(sw.SweError) as e:
         sw.swe_mesh_create(x, y, z, np.array([[0, 1, 2]], np.int32), renumber=5)
     assert e.value.code == sw.SWE_ERR_ARG
+
+
+def test_graph_replay_equals_kernel_by_kernel_launches():
+    """swe_step replays one captured CUDA graph per step (nsteps >= 2): same kernels, same order --
+    the state, the clock and the launch count must be those of the plain launches, through scheme
+    changes, parameter changes and zones (each invalidates the captured graph)."""
+    cfg = _river()
+    a = sw.create_from_config(cfg)
+    b = sw.create_from_config(cfg)
+    try:
+        sw.swe_set_graphs(b, False)
+        seq = [("muscl", 0.45, 12), ("hllc", 0.9, 7), ("muscl", 0.45, 1), ("waf", 0.45, 5), ("muscl", 0.3, 6),
+               ("muscl_ms", 0.45, 4)]
+        for x in (a, b):
+            for scheme, cfl, n in seq:
+                t = sw.swe_step(x, n, cfl, scheme)
+            sw.swe_set_params(x, beta=2.0)
+            sw.swe_step(x, 5, 0.45, "muscl")
+            sw.swe_zones_create(x, 8, 2)
+            sw.swe_step(x, 6, 0.45, "muscl")
+            sw.swe_step(x, 3, 0.9, "hllc")
+            sw.swe_zones_create(x, 0, 1)
+            sw.swe_step(x, 4, 0.45, "muscl")
+        for u, v in zip(sw.swe_get_state(a), sw.swe_get_state(b)):
+            assert np.array_equal(u, v)
+        assert sw.swe_get_time(a) == sw.swe_get_time(b)
+        sa, sb = sw.swe_get_stats(a), sw.swe_get_stats(b)
+        assert sa == sb
+    finally:
+        sw.swe_mesh_destroy(a)
+        sw.swe_mesh_destroy(b)
