@@ -28,13 +28,12 @@
 // conserved to round-off without a flux buffer.  No blocking, fusion or reordering.
 //
 // The open boundaries (inflow Q: sign, magnitude, distribution over the tag's width; fixed level:
-// ghost depth) are pinned by tests/test_oracle_boundaries.py (uniform flow preserved to round-off,
-// relaxation to the backwater curve of the gradually-varied-flow ODE).
+// ghost depth and outgoing Riemann invariant) are pinned by tests/test_oracle_boundaries.py
+// (uniform flow preserved to round-off, relaxation to the backwater curve of the
+// gradually-varied-flow ODE, reflection of a small long wave with coefficient -1).
 // PARITY UNPINNED (only oracle<->GPU agreement and mass balance check these):
-//   the transient behaviour of the fixed-level boundary (the choice of the outgoing Riemann
-//   invariant for its normal velocity; at a steady state any consistent choice gives the same
-//   result), the momentum part of the inflow flux on dry faces, the WAF Delta-x choice on
-//   triangles, the values of h_dry / h_thin, the WAF->HLLC fallback rule.
+//   the momentum part of the inflow flux on dry faces, the WAF Delta-x choice on triangles, the
+//   values of h_dry / h_thin, the WAF->HLLC fallback rule.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>

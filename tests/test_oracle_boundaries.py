@@ -91,3 +91,34 @@ def test_backwater_reference_is_the_textbook_curve():
     x_of_h = L + np.concatenate([[0.0], np.cumsum(0.5 * (dxdh[1:] + dxdh[:-1]) * np.diff(hs))])
     for k in (500, 2000, 4000):
         assert abs(_backwater(np.array([x_of_h[k]]), q, n, level, L)[0] - hs[k]) < 1e-6
+
+
+@pytest.mark.parametrize("scheme,cfl,keep", [("muscl", 0.45, 0.9), ("hllc", 0.9, 0.8), ("waf", 0.45, 0.85),
+                                             ("muscl_ms", 0.45, 0.85)])
+def test_fixed_level_boundary_reflects_with_coefficient_minus_one(scheme, cfl, keep, oracle_threads):
+    """Transient behaviour of the fixed-level boundary (the outgoing Riemann invariant of R11):
+    linear theory -- a boundary that holds the free surface reflects a small long wave with
+    coefficient -1 in elevation and +1 in velocity.  A right-running simple-wave pulse of amplitude
+    a = 1 cm on h0 = 1 m, centred at x0 = 60 m, comes back inverted: after t = (100 - x0)/c +
+    50/c its trough sits at x = 50 m with eta = -a and u = +a c / h0 (less the scheme's damping).
+    A wall-like treatment, or the invariant with the wrong sign, returns a crest instead."""
+    h0, a, x0, w = 1.0, 0.01, 60.0, 6.0
+    cfg = si.channel_flow_case(nx=400, ny=4, lx=100.0, ly=1.0, jitter=0.1, discharge=0.0, level=h0)
+    cx = cfg["x"][cfg["tri"]].mean(axis=1)
+    h = h0 + a * np.exp(-((cx - x0) / w) ** 2)
+    cfg["h"] = h
+    cfg["hu"] = h * 2.0 * (np.sqrt(G * h) - np.sqrt(G * h0))       # right-running simple wave
+    o = po.Oracle.from_config(cfg)
+    c = np.sqrt(G * h0)
+    T = (100.0 - x0) / c + 50.0 / c
+    t, _ = o.step(int(0.98 * T / o.compute_dt(cfl)), cfl, scheme)   # dt is almost constant (a << h0)
+    while t < T:
+        t, _ = o.step(1, cfl, scheme)
+    hh, hu, hv = o.get_state()
+    eta = hh - h0
+    i = int(np.argmin(eta))
+    assert -1.02 * a < eta[i] < -keep * a                  # inverted, amplitude kept up to the damping
+    assert abs(cx[i] - 50.0) < 3.0                         # where linear theory puts it
+    assert eta.max() < 0.05 * a                            # no crest comes back
+    u = hu[i] / hh[i]
+    assert keep * a * c / h0 < u < 1.05 * a * c / h0       # velocity perturbation keeps its sign
