@@ -148,6 +148,31 @@ def test_ranks_in_one_process_bit_identical(transport, overlap, world, nz, nl, s
         R.close()
 
 
+def test_config3_full_size_two_ranks_overlap_schedule():
+    """The workload bench.py runs at N = 2 (configs[3], 13.1 M cells, 2 zones over 2 ranks, 2 ghost
+    layers, peer-memory push, overlap schedule), ranks in one process: 3 MUSCL-RK2 steps
+    bit-identical to the single-GPU run."""
+    from swe_inputs import config3 as full
+    cfg = full()
+    a = sw.create_from_config(cfg)
+    try:
+        ta = sw.swe_step(a, 3, 0.45, "muscl")
+        ref = sw.swe_get_state(a)
+    finally:
+        sw.swe_mesh_destroy(a)
+    R = _Ranks(cfg, 2, 2, 2, "p2p")
+    try:
+        R.step(3, 0.45, "muscl", overlap=True)
+        got = R.state(ref[0].size)
+        for x, y in zip(ref, got):
+            assert np.array_equal(x, y)
+        assert sw.swe_get_time(R.ctx[1]) == ta
+        s, r = R.counts[0]
+        assert s[1] == r[1] and 1000 < s[1] < 100000        # a few thousand cells cross the cut
+    finally:
+        R.close()
+
+
 def test_one_layer_hllc_and_errors():
     cfg = _river()
     a = sw.create_from_config(cfg)
