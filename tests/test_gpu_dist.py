@@ -168,7 +168,7 @@ def test_config3_full_size_two_ranks_overlap_schedule():
             assert np.array_equal(x, y)
         assert sw.swe_get_time(R.ctx[1]) == ta
         s, r = R.counts[0]
-        assert s[1] == r[1] and 1000 < s[1] < 100000        # a few thousand cells cross the cut
+        assert s[1] == r[1] and 500 < s[1] < 100000          # two layers of the cells along the cut
     finally:
         R.close()
 
