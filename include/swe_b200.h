@@ -135,7 +135,9 @@ int swe_zone_sendlist(const swe_ctx* ctx, int zone, int link, int32_t* send_idx)
  * swe_set_state / swe_set_manning / swe_set_bc are called on every rank with the same full-mesh
  * arguments; swe_get_state writes only the cells owned by this rank's zones and leaves the other
  * entries of the output arrays untouched.  nlayers >= 2 is required for MUSCL, WAF and MUSCL_MS
- * (no gradient exchange between ranks); nlayers = 1 serves HLLC.
+ * (no gradient exchange between ranks); nlayers = 1 serves HLLC.  Removing the zones again
+ * (swe_zones_create(ctx, 0, ..)) brings back only the cells this rank owned: call swe_set_state with
+ * the gathered full state before stepping un-zoned.
  *   zone_begin : nranks+1 non-decreasing zone ids from 0 to nzones (host pointer); may be NULL when
  *                nranks == 1.  Errors: SWE_ERR_ARG. */
 int swe_zones_create_dist(swe_ctx* ctx, int nzones, int nlayers, const int32_t* zone_of_cell,
