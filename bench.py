@@ -298,6 +298,7 @@ def main():
     ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--renumber", default="hilbert", choices=["hilbert", "rcm", "none"])
     ap.add_argument("--transport", default="p2p", choices=["p2p", "staged"])
     ap.add_argument("--schedule", default="overlap", choices=["overlap", "plain"])
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
@@ -324,7 +325,8 @@ def main():
     cfl = 0.9 if args.scheme == "hllc" else 0.45
     if world > 1 and not args.replicas:
         return run_dist(args, rank, world, local, cfg, desc, cfl)
-    ctx = sw.create_from_config(cfg)
+    ctx = sw.create_from_config(cfg, {"hilbert": sw.SWE_RENUM_HILBERT, "rcm": sw.SWE_RENUM_RCM,
+                                      "none": sw.SWE_RENUM_NONE}[args.renumber])
     info = sw.swe_mesh_info(ctx)
     nt = info["ncell"]
     if args.zones > 0:
@@ -394,7 +396,8 @@ def main():
                        "l2": "inputs larger than L2 (state+geometry+flux > 3 GB per stage at 13 M cells)"
                        if nt > 2_000_000 else "working set may fit L2 at this size",
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
-                       "zones": args.zones, "ghost_layers": args.layers if args.zones else 0},
+                       "zones": args.zones, "ghost_layers": args.layers if args.zones else 0,
+                       "renumber": args.renumber},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
             "gpu_launches": l1["kernel_launches"] - l0["kernel_launches"], "clocks": clocks,
         }

@@ -49,7 +49,9 @@ enum { SWE_OK = 0, SWE_ERR_ARG = -1, SWE_ERR_MESH = -2, SWE_ERR_CUDA = -3, SWE_E
 enum { SWE_HLLC = 0, SWE_MUSCL = 1, SWE_WAF = 2, SWE_MUSCL_MS = 3 };
 /* boundary kinds (fixed level: PAPER.md:518, 548, reading R11) */
 enum { SWE_BC_WALL = 0, SWE_BC_INFLOW_Q = 1, SWE_BC_LEVEL = 2, SWE_BC_TRANSMISSIVE = 3 };
-enum { SWE_RENUM_NONE = 0, SWE_RENUM_HILBERT = 1 };
+/* cell renumbering for gather locality (north_star): Hilbert curve through the centroids, or reverse
+ * Cuthill-McKee over the edge adjacency.  Results do not depend on it (orientation by user id). */
+enum { SWE_RENUM_NONE = 0, SWE_RENUM_HILBERT = 1, SWE_RENUM_RCM = 2 };
 
 /* Build the mesh (host: topology + geometry of SURVEY.md Appendix A.1, renumbering; then upload).
  *   nv, x, y, zb : vertices, coordinates [m] and bed elevation [m] per vertex

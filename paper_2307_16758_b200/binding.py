@@ -16,7 +16,7 @@ SWE_OK = 0
 SWE_ERR_ARG, SWE_ERR_MESH, SWE_ERR_CUDA, SWE_ERR_STATE, SWE_ERR_NOMEM = -1, -2, -3, -4, -5
 SWE_HLLC, SWE_MUSCL, SWE_WAF, SWE_MUSCL_MS = 0, 1, 2, 3
 SWE_BC_WALL, SWE_BC_INFLOW_Q, SWE_BC_LEVEL, SWE_BC_TRANSMISSIVE = 0, 1, 2, 3
-SWE_RENUM_NONE, SWE_RENUM_HILBERT = 0, 1
+SWE_RENUM_NONE, SWE_RENUM_HILBERT, SWE_RENUM_RCM = 0, 1, 2
 SCHEMES = {"hllc": SWE_HLLC, "muscl": SWE_MUSCL, "waf": SWE_WAF, "muscl_ms": SWE_MUSCL_MS}
 BC_KINDS = {"wall": SWE_BC_WALL, "inflow": SWE_BC_INFLOW_Q, "level": SWE_BC_LEVEL,
             "transmissive": SWE_BC_TRANSMISSIVE}

@@ -165,6 +165,56 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         std::sort(cell_user.begin(), cell_user.end(), [&](int32_t a, int32_t b) {
             return key[a] != key[b] ? key[a] < key[b] : a < b; });
     }
+    // ---- or reverse Cuthill-McKee over the edge adjacency (north_star: "space-filling-curve or RCM
+    // pass"): per connected component, root = a minimum-degree cell of the last level of a
+    // breadth-first search from the component's lowest user id; neighbours by (degree, user id) ----
+    if (renumber == 2 && nt > 1) {
+        auto nbr = [&](int32_t u, int k) -> int32_t {
+            const int32_t e = side_edge[3 * (int64_t)u + k];
+            const int32_t L = esL[e] / 3, R = esR[e] >= 0 ? esR[e] / 3 : -1;
+            return L == u ? R : L;
+        };
+        std::vector<uint8_t> deg(nt, 0), seen(nt, 0), done(nt, 0);
+        for (int64_t u = 0; u < nt; ++u)
+            for (int k = 0; k < 3; ++k) if (nbr((int32_t)u, k) >= 0) deg[u]++;
+        std::vector<int32_t> order; order.reserve(nt);
+        std::vector<int32_t> q;
+        for (int64_t s0 = 0; s0 < nt; ++s0) {
+            if (done[s0]) continue;
+            // level structure from s0: the last level's minimum-degree cell becomes the root
+            q.assign(1, (int32_t)s0); seen[s0] = 1;
+            size_t lstart = 0, lend = 1;
+            for (;;) {
+                lend = q.size();
+                for (size_t h2 = lstart; h2 < lend; ++h2)
+                    for (int k = 0; k < 3; ++k) {
+                        const int32_t v = nbr(q[h2], k);
+                        if (v >= 0 && !seen[v]) { seen[v] = 1; q.push_back(v); }
+                    }
+                if (q.size() == lend) break;                  // [lstart, lend) is the last level
+                lstart = lend;
+            }
+            int32_t root = q[lstart];
+            for (size_t j = lstart; j < lend; ++j)
+                if (deg[q[j]] < deg[root] || (deg[q[j]] == deg[root] && q[j] < root)) root = q[j];
+            // Cuthill-McKee from the root
+            const size_t first = order.size();
+            order.push_back(root); done[root] = 1;
+            for (size_t h2 = first; h2 < order.size(); ++h2) {
+                const int32_t u = order[h2];
+                int32_t cand[3]; int nc2 = 0;
+                for (int k = 0; k < 3; ++k) {
+                    const int32_t v = nbr(u, k);
+                    if (v >= 0 && !done[v]) { done[v] = 1; cand[nc2++] = v; }
+                }
+                auto before = [&](int32_t a, int32_t b) { return deg[a] != deg[b] ? deg[a] < deg[b] : a < b; };
+                for (int a = 1; a < nc2; ++a)                  // insertion sort of at most 3
+                    for (int b = a; b > 0 && before(cand[b], cand[b - 1]); --b) std::swap(cand[b], cand[b - 1]);
+                for (int j = 0; j < nc2; ++j) order.push_back(cand[j]);
+            }
+        }
+        for (int64_t i = 0; i < nt; ++i) cell_user[i] = order[nt - 1 - i];      // reversed
+    }
     H.user_cell.resize(nt);
     for (int64_t i = 0; i < nt; ++i) H.user_cell[cell_user[i]] = (int32_t)i;
 

@@ -410,7 +410,7 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     *out = nullptr;
     if (nv <= 0 || nt <= 0 || !x || !y || !zb || !tri) return fail(SWE_ERR_ARG, "empty or NULL mesh arrays");
     if (nb < 0 || (nb > 0 && (!bedge || !btag))) return fail(SWE_ERR_ARG, "bad boundary-edge arguments");
-    if (renumber != SWE_RENUM_NONE && renumber != SWE_RENUM_HILBERT) return fail(SWE_ERR_ARG, "unknown renumbering");
+    if (renumber != SWE_RENUM_NONE && renumber != SWE_RENUM_HILBERT && renumber != SWE_RENUM_RCM) return fail(SWE_ERR_ARG, "unknown renumbering");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();

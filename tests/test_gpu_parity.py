@@ -113,21 +113,24 @@ def test_per_step_and_run_parity_small(name, scheme, cfl):
 
 
 def test_renumbering_is_invisible():
-    """Hilbert and identity numbering give bit-identical results (orientation, summation order and
+    """Hilbert, reverse Cuthill-McKee and identity numbering give bit-identical results (orientation, summation order and
     dt do not depend on the internal numbering)."""
     cfg = _small_cases()["river"]
     a = sw.create_from_config(cfg, sw.SWE_RENUM_NONE)
     b = sw.create_from_config(cfg, sw.SWE_RENUM_HILBERT)
+    r = sw.create_from_config(cfg, sw.SWE_RENUM_RCM)
     try:
         for scheme, cfl in (("muscl", 0.45), ("waf", 0.45), ("hllc", 0.9), ("muscl_ms", 0.45)):
             ta = sw.swe_step(a, 25, cfl, scheme)
             tb = sw.swe_step(b, 25, cfl, scheme)
-            assert ta == tb
-            for x, y in zip(sw.swe_get_state(a), sw.swe_get_state(b)):
-                assert np.array_equal(x, y)
+            tr = sw.swe_step(r, 25, cfl, scheme)
+            assert ta == tb == tr
+            for x, y, z in zip(sw.swe_get_state(a), sw.swe_get_state(b), sw.swe_get_state(r)):
+                assert np.array_equal(x, y) and np.array_equal(x, z)
     finally:
         sw.swe_mesh_destroy(a)
         sw.swe_mesh_destroy(b)
+        sw.swe_mesh_destroy(r)
 
 
 # ---------------------------------------------------------------------------------------------

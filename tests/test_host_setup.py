@@ -45,7 +45,7 @@ def _cases():
 
 
 @pytest.mark.parametrize("name", ["c0", "c1", "lake", "river"])
-@pytest.mark.parametrize("renum", [sw.SWE_RENUM_NONE, sw.SWE_RENUM_HILBERT])
+@pytest.mark.parametrize("renum", [sw.SWE_RENUM_NONE, sw.SWE_RENUM_HILBERT, sw.SWE_RENUM_RCM])
 def test_host_mesh_matches_oracle_geometry(name, renum):
     cfg = _cases()[name]
     o = po.Oracle.from_config(cfg)
@@ -216,3 +216,23 @@ def test_mesh_errors():
     with pytest.raises(sw.SweError):
         sw.swe_host_zones_build(h, 2, 4)      # nlayers in 1..3
     sw.swe_host_mesh_free(h)
+
+
+def test_rcm_order_has_a_small_bandwidth():
+    """Reverse Cuthill-McKee: neighbours get close numbers.  On the permuted configs[1] mesh the
+    identity numbering has a bandwidth of the order of the cell count; RCM brings it down to the
+    order of the number of cells across the domain."""
+    from swe_inputs import config1
+    cfg = config1(n=60)
+    nt = cfg["tri"].shape[0]
+    bw = {}
+    for renum in (sw.SWE_RENUM_NONE, sw.SWE_RENUM_RCM, sw.SWE_RENUM_HILBERT):
+        h = sw.swe_host_mesh_build(cfg["x"], cfg["y"], cfg["zb"], cfg["tri"], cfg["bedge"], cfg["btag"], renum)
+        c2c = sw.swe_host_get(h, "c2c").reshape(-1, 4)[:, :3]
+        i = np.repeat(np.arange(nt), 3).reshape(-1, 3)
+        d = np.abs(c2c - i)[c2c >= 0]
+        bw[renum] = (int(d.max()), float(d.mean()))
+        sw.swe_host_mesh_free(h)
+    assert bw[sw.SWE_RENUM_NONE][0] > nt // 2
+    assert bw[sw.SWE_RENUM_RCM][0] < 6 * 60                  # a few rows of the 60 x 60 x 2 mesh
+    assert bw[sw.SWE_RENUM_RCM][1] < 0.05 * bw[sw.SWE_RENUM_NONE][1]
