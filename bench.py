@@ -43,6 +43,9 @@ def build_workload(name):
     from swe_inputs import config1, config2, config3
     if name == "c3":
         return config3(), "configs[3]: 60 km x 8 km synthetic river mesh, ~13 M triangles, seed 3"
+    if name == "c3p":
+        from swe_inputs import permuted
+        return permuted(config3()), "configs[3] with its ~13 M triangles listed in a random order (seed 7)"
     if name == "c3s":
         return config3(length=6000.0), "configs[3] generator on a 6 km reach (~1.3 M triangles), seed 3"
     if name == "c3t":
@@ -294,7 +297,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3s", "c3t", "c1", "c2"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3p", "c3s", "c3t", "c1", "c2"])
     ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)

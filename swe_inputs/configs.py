@@ -158,6 +158,20 @@ def simple_wave_case(nx, ny=None, lx=100.0, ly=None, jitter=0.0, seed=0, h0=1.0,
     return cfg
 
 
+def permuted(cfg, seed=7):
+    """The same case with its triangles listed in a random order (as a mesh generator or a
+    partitioner may hand them over): tri and every per-cell field are permuted together."""
+    rng = np.random.default_rng(seed)
+    p = rng.permutation(cfg["tri"].shape[0])
+    out = dict(cfg)
+    out["tri"] = np.ascontiguousarray(cfg["tri"][p])
+    for k in ("h", "hu", "hv", "manning"):
+        if cfg.get(k) is not None:
+            out[k] = np.ascontiguousarray(cfg[k][p])
+    out["name"] = cfg["name"] + "_permuted"
+    return out
+
+
 def channel_flow_case(nx=100, ny=5, lx=100.0, ly=5.0, jitter=0.1, seed=4, discharge=10.0, level=2.0,
                       manning=0.0, h_init=None, u_init=0.0):
     """Straight flat channel with the two open boundaries of configs[3]: imposed discharge Q on the
