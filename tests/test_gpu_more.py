@@ -5,7 +5,7 @@ import pytest
 
 import paper_2307_16758_b200 as sw
 from oracle import pyoracle as po
-from swe_inputs import config0, config3, simple_wave_case, lake_case
+from swe_inputs import config0, config3, simple_wave_case, lake_case, channel_flow_case
 from parity import assert_parity
 
 pytestmark = pytest.mark.gpu
@@ -61,6 +61,46 @@ def test_boundary_kinds(kinds, scheme, cfl):
     finally:
         sw.swe_mesh_destroy(c)
         o.close()
+
+
+@pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_open_channel_flow_free_run(scheme, cfl):
+    """The case that pins the oracle's open boundaries (tests/test_oracle_boundaries.py): inflow Q,
+    fixed level, Manning friction, relaxing from still water towards the backwater curve -- a free
+    run of 400 steps on the GPU stays within 1e-8 of the oracle, and the GPU keeps the uniform flow
+    exactly as the oracle does.  WAF: 100 steps -- on this case the per-edge WAF with SUPERBEE
+    amplifies round-off tenfold every 25 steps (both sides agree to 3e-16 when restarted every step;
+    free trajectories are 2e-12 apart after 100 steps, 5e-8 after 200, 1e-2 after 400: DESIGN.md 3)."""
+    cfg = channel_flow_case(nx=100, ny=5, lx=200.0, ly=10.0, discharge=20.0, level=1.0, manning=0.03)
+    o = po.Oracle.from_config(cfg)
+    c = sw.create_from_config(cfg)
+    try:
+        if scheme == "waf":                              # every step from the oracle's state: 1e-11
+            for s in range(150):
+                sw.swe_set_state(c, *o.get_state())
+                o.step(1, cfl, scheme)
+                sw.swe_step(c, 1, cfl, scheme)
+                assert_parity(o.get_state(), sw.swe_get_state(c), 1e-11, what="channel waf step %d" % s)
+            o.close()
+            o = po.Oracle.from_config(cfg)               # and a free run from the start
+            sw.swe_set_state(c, cfg["h"], cfg["hu"], cfg["hv"])
+            sw.swe_set_time(c, 0.0)
+        n = 100 if scheme == "waf" else 400
+        to = o.step(n, cfl, scheme)
+        tg = sw.swe_step(c, n, cfl, scheme)
+        assert abs(to[0] - tg[0]) <= 1e-10 * to[0]
+        assert_parity(o.get_state(), sw.swe_get_state(c), 1e-8, what="channel " + scheme)
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+    cfg = channel_flow_case(discharge=10.0, level=2.0, u_init=1.0)
+    c = sw.create_from_config(cfg)
+    try:
+        sw.swe_step(c, 200, cfl, scheme)
+        h, hu, hv = sw.swe_get_state(c)
+        assert np.abs(h - 2.0).max() < 1e-13 and np.abs(hu - 2.0).max() < 1e-13 and np.abs(hv).max() < 1e-13
+    finally:
+        sw.swe_mesh_destroy(c)
 
 
 @pytest.mark.parametrize("beta", [2.0, 1.0])
