@@ -198,7 +198,15 @@ def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workloa
     traffic = tt.get((workload, dom + "_" + scheme), tt.get((workload, dom)))
     step_bytes = ALGO_BYTES["step_" + scheme]
     rate = cells / (step_ms * 1e-3)
-    return {
+    # physical DRAM bytes of one step from the ncu table (13.1 M-cell MUSCL-RK2 only), SURVEY 8(d)(iii)
+    step_dram = None
+    if scheme == "muscl" and all((workload, k) in tt for k in ("grad_limit", "edge_flux_muscl", "cell_update_muscl")):
+        step_dram = 2.0 * (tt[(workload, "grad_limit")] + tt[(workload, "edge_flux_muscl")] + tt[(workload, "cell_update_muscl")])
+    extra = {}
+    if step_dram:
+        extra = {"step_dram_bytes_ncu": step_dram, "step_algo_over_dram_bytes": step_bytes * cells / step_dram,
+                 "step_dram_GBps": step_dram / (step_ms * 1e-3) / 1e9}
+    return dict(extra, **{
         "bound": "hbm", "kernel": dom, "achieved": kern[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
         "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
         "algo_bytes_per_launch": algo[dom] * cells,
@@ -206,7 +214,7 @@ def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workloa
         "step_frac_of_peak": step_bytes * rate / 1e9 / peak,
         "step_frac_of_8TBps": step_bytes * rate / 1e9 / 8000.0,
         "kernels": kern,
-    }
+    })
 
 
 def run_dist(args, rank, world, local, cfg, desc, cfl):
