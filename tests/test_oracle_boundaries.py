@@ -122,3 +122,34 @@ def test_fixed_level_boundary_reflects_with_coefficient_minus_one(scheme, cfl, k
     assert eta.max() < 0.05 * a                            # no crest comes back
     u = hu[i] / hh[i]
     assert keep * a * c / h0 < u < 1.05 * a * c / h0       # velocity perturbation keeps its sign
+
+
+@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_inflow_onto_a_dry_bed_fills_the_channel_with_Q_t(scheme, cfl, oracle_threads):
+    """Imposed discharge onto a dry bed (reading R10): whatever the momentum part of the boundary flux
+    on a dry face, the mass part is q_n = -Q / W on every tagged edge, so a closed channel holds
+    exactly Q t of water after time t (to round-off), depths never go negative, and the water has
+    got as far as a front moving at a few m/s can -- not further, not nowhere.  (The pool is 0.5 m
+    deep: with a 5 cm film the inflow is a Froude-17 jet, the second Heun stage -- which uses the
+    dt of U^n, A.2 -- overshoots, and the clamp h' = max(h', 0) of A.10 creates mass in the first
+    steps of MUSCL / MUSCL_MS, 0.24 m3 here; HLLC and WAF stay exact.  DESIGN.md, tolerances.)"""
+    Q, lx, ly = 3.0, 100.0, 5.0
+    cfg = si.channel_flow_case(nx=200, ny=10, lx=lx, ly=ly, discharge=Q, level=0.0, h_init=0.0)
+    cfg["bc"] = {1: ("inflow", Q), 2: ("wall", 0.0)}
+    o = po.Oracle.from_config(cfg)
+    assert o.compute_dt(cfl) == 0.0                        # nothing is wet yet: dt = 0, the step is a no-op
+    # a pool next to the inlet gets the clock going (its volume is accounted for)
+    import closed_forms as cf
+    cx = cfg["x"][cfg["tri"]].mean(axis=1)
+    area = cf.tri_areas(cfg["x"], cfg["y"], cfg["tri"])
+    h0 = np.where(cx < 4.0, 0.5, 0.0)
+    o.set_state(h0, np.zeros_like(h0), np.zeros_like(h0))
+    v0 = float((h0 * area).sum())
+    t, _ = o.step(600, cfl, scheme)
+    h, hu, hv = o.get_state()
+    assert h.min() >= 0.0
+    vol = float((h * area).sum())
+    assert abs(vol - (v0 + Q * t)) < 1e-11 * (v0 + Q * t)
+    front = cx[h > 1e-3].max()
+    assert 5.0 < front and (front < lx - 1.0 or t > 10.0)
+    assert t > 1.0
