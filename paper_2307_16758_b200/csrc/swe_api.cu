@@ -333,12 +333,13 @@ void run_update(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, do
         const int n = (int)c->nsendcells;
         if (n == 0) return;
         launch(c, KIND_UPDATE, [&] {
-            const int gr = grid_for(n, c->grid_light);
+            // a few thousand cells: 64-thread blocks spread them over the SMs (a latency-bound launch)
+            const int gr = grid_for(n, c->grid_light * 4, 64);
             const int* L = c->d_send_cells;
-            if (mode == 0 && !fuse) k_cell_update_list<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
-            else if (mode == 0) k_cell_update_list<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
-            else if (!fuse) k_cell_update_list<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
-            else k_cell_update_list<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            if (mode == 0 && !fuse) k_cell_update_list<0, false><<<gr, 64, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else if (mode == 0) k_cell_update_list<0, true><<<gr, 64, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else if (!fuse) k_cell_update_list<1, false><<<gr, 64, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
+            else k_cell_update_list<1, true><<<gr, 64, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, L, n);
         });
         return;
     }
@@ -1036,7 +1037,7 @@ int swe_halo_push(swe_ctx* c, int buffer) {
     double4* U = buffer ? c->z.B : c->z.A;
     if (c->nrsend) {
         launch(c, KIND_PACK, [&] {
-            k_halo_push<<<grid_for(c->nrsend, c->grid_light), 256, 0, c->stream>>>(U, c->d_rsend_idx, c->d_rsend_dst, c->d_rsend_peer,
+            k_halo_push<<<grid_for(c->nrsend, c->grid_light * 4, 64), 64, 0, c->stream>>>(U, c->d_rsend_idx, c->d_rsend_dst, c->d_rsend_peer,
                                                                                   buffer ? c->d_peerB : c->d_peerA, c->nrsend);
         });
         c->halo_bytes += c->nrsend * (12 + 32 + 32);
