@@ -46,6 +46,9 @@ def build_workload(name):
     if name == "c3p":
         from swe_inputs import permuted
         return permuted(config3()), "configs[3] with its ~13 M triangles listed in a random order (seed 7)"
+    if name == "c3w":
+        from swe_inputs import flooded
+        return flooded(config3(), 18.0), "configs[3] mesh and bed, flooded to a flat surface at 18 m: no dry cell"
     if name == "c3s":
         return config3(length=6000.0), "configs[3] generator on a 6 km reach (~1.3 M triangles), seed 3"
     if name == "c3t":
@@ -309,7 +312,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3p", "c3s", "c3t", "c1", "c2"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3p", "c3w", "c3s", "c3t", "c1", "c2"])
     ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)

@@ -9,8 +9,8 @@ depth = max(0, level - bed)).  Recipes are stated in DESIGN.md ("Input recipe").
 from .meshes import grid_mesh, river_mesh, boundary_edges
 from .noise import value_noise, gaussian_bumps
 from .configs import (config0, config1, config2, config3, simple_wave_case, lake_case,
-                      channel_flow_case, permuted, CONFIG_BUILDERS)
+                      channel_flow_case, permuted, flooded, CONFIG_BUILDERS)
 
 __all__ = ["grid_mesh", "river_mesh", "boundary_edges", "value_noise", "gaussian_bumps",
            "config0", "config1", "config2", "config3", "simple_wave_case", "lake_case",
-           "channel_flow_case", "permuted", "CONFIG_BUILDERS"]
+           "channel_flow_case", "permuted", "flooded", "CONFIG_BUILDERS"]

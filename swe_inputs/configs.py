@@ -172,6 +172,18 @@ def permuted(cfg, seed=7):
     return out
 
 
+def flooded(cfg, level):
+    """The same case with a flat free surface at `level` (above every cell's bed where level is
+    high enough): no dry cells, velocity zero.  depth = max(0, level - cell bed)."""
+    out = dict(cfg)
+    zc = _cell_bed(cfg["zb"], cfg["tri"])
+    out["h"] = np.ascontiguousarray(np.maximum(0.0, level - zc))
+    out["hu"] = np.zeros_like(out["h"])
+    out["hv"] = np.zeros_like(out["h"])
+    out["name"] = cfg["name"] + "_flooded"
+    return out
+
+
 def channel_flow_case(nx=100, ny=5, lx=100.0, ly=5.0, jitter=0.1, seed=4, discharge=10.0, level=2.0,
                       manning=0.0, h_init=None, u_init=0.0):
     """Straight flat channel with the two open boundaries of configs[3]: imposed discharge Q on the
