@@ -394,6 +394,7 @@ def main():
            "h2d_bytes_per_step": 3 * 8 * nt, "d2h_bytes_per_step": 3 * 8 * nt,
            "what": "per step: swe_set_state(pinned host) + swe_step(1) + swe_get_state(pinned host)"}
     zstats = sw.swe_zone_stats(ctx) if args.zones > 0 else None
+    roofline["fp64_peak_TFLOPs_measured"] = sw.swe_fp64_peak(ctx)      # the other side of the roofline
     sw.swe_mesh_destroy(ctx)
 
     # ---- the oracle as it stands, timed on this box's host cores (rank 0, N=1 only) ----

@@ -214,6 +214,10 @@ int swe_get_stats(const swe_ctx* ctx, int64_t* steps, int64_t* kernel_launches, 
 /* time the hot path with CUDA events on the context's stream: runs swe_step(nsteps,...) between
  * two events and returns the elapsed milliseconds (synchronises). */
 int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_out);
+/* fp64 FMA throughput of the device in TFLOP/s (2 flops per FMA; eight independent chains per
+ * thread, 8 blocks of 256 threads per SM, best of 3 timed launches): the ALU-side roofline the
+ * bandwidth-bound claim is checked against.  Synchronises. */
+int swe_fp64_peak(swe_ctx* ctx, double* tflops_out);
 /* per-kernel timing: runs `reps` launches of one kernel of the hot path on the current state
  * between two events; which: 0 dt_reduce, 1 grad_limit, 2 edge_flux(scheme), 3 cell_update (Euler
  * stage), 4 cell_update (Heun combine), 5 pack, 6 unpack.  The state is left unchanged (updates

@@ -38,6 +38,7 @@ SIGNATURES = {
     "swe_set_time": (C.c_int, [_vp, C.c_double]),
     "swe_step": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, _dp, _dp]),
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
+    "swe_fp64_peak": (C.c_int, [_vp, _dp]),
     "swe_zones_create": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_unpack_ghosts": (C.c_int, [_vp, C.c_int]),
@@ -198,6 +199,12 @@ def swe_step(ctx, nsteps, cfl, scheme, sync=True):
     t, dt = C.c_double(), C.c_double()
     _check(lib().swe_step(ctx, int(nsteps), float(cfl), _scheme(scheme), C.byref(t), C.byref(dt)))
     return t.value, dt.value
+
+
+def swe_fp64_peak(ctx):
+    v = C.c_double()
+    _check(lib().swe_fp64_peak(ctx, C.byref(v)))
+    return v.value
 
 
 def swe_set_graphs(ctx, on):

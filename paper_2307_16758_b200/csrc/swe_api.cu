@@ -683,6 +683,31 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
     return SWE_OK;
 }
 
+int swe_fp64_peak(swe_ctx* c, double* tflops_out) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!tflops_out) return fail(SWE_ERR_ARG, "NULL output");
+    const int blocks = c->num_sm * 8, iters = 2048;
+    double* d = nullptr;
+    CU(cudaMalloc((void**)&d, (size_t)blocks * 256 * sizeof(double)));
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {                 // first repetition warms up
+        cudaEventRecord(a, c->stream);
+        k_dfma_peak<<<blocks, 256, 0, c->stream>>>(d, iters);
+        cudaEventRecord(b, c->stream);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(d);
+    CU(cudaGetLastError());
+    *tflops_out = 2.0 * 32.0 * (double)iters * blocks * 256 / (best * 1e-3) / 1e12;
+    return SWE_OK;
+}
+
 int swe_set_graphs(swe_ctx* c, int on) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     c->use_graphs = on != 0;

@@ -319,3 +319,14 @@ def test_graph_replay_equals_kernel_by_kernel_launches():
     finally:
         sw.swe_mesh_destroy(a)
         sw.swe_mesh_destroy(b)
+
+
+def test_fp64_peak_microbenchmark():
+    """The DFMA micro-benchmark BASELINE.md asks for: a plausible B200 figure (tens of TFLOP/s)."""
+    c = sw.create_from_config(config0())
+    try:
+        v = sw.swe_fp64_peak(c)
+        assert 10.0 < v < 100.0, v
+        assert abs(sw.swe_fp64_peak(c) - v) < 0.2 * v
+    finally:
+        sw.swe_mesh_destroy(c)
