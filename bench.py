@@ -134,10 +134,10 @@ def traffic_table():
     return out
 
 
-def oracle_run(cfg, scheme, cfl, warmup, steps, budget_s=None):
-    """Times the CPU oracle as it stands (all host cores); returns cell-updates/s and details."""
+def oracle_run(cfg, scheme, cfl, warmup, steps, budget_s=None, threads=0):
+    """Times the CPU oracle as it stands (threads = 0: all host cores); returns cell-updates/s and details."""
     from oracle import pyoracle as po
-    cores = po.set_threads(0)
+    cores = po.set_threads(threads)
     o = po.Oracle.from_config(cfg)
     t0 = time.perf_counter()
     o.step(max(1, warmup), cfl, scheme)
@@ -403,8 +403,10 @@ def main():
         sname = "c3s" if args.workload == "c3" else args.workload
         scfg, sdesc = (cfg, desc) if sname == args.workload else build_workload(sname)
         v, cores, ont, secs, osteps = oracle_run(scfg, args.scheme, cfl, 1, 400, budget_s=15.0)
+        v1, _, _, secs1, osteps1 = oracle_run(scfg, args.scheme, cfl, 1, 50, budget_s=5.0, threads=1)
         cpu_baseline = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle",
-                        "sample": "%s: %d cells x %d %s steps in %.1f s" % (sdesc, ont, osteps, args.scheme, secs)}
+                        "sample": "%s: %d cells x %d %s steps in %.1f s" % (sdesc, ont, osteps, args.scheme, secs),
+                        "single_thread": {"value": v1, "cores": 1, "sample": "%d steps in %.1f s" % (osteps1, secs1)}}
 
     if rank == 0:
         line = {
