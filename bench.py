@@ -36,6 +36,16 @@ ALGO_BYTES = {  # algorithmic bytes per cell (N_e = 1.5 
     "edge_flux_muscl_ms": 200.0, "step_muscl_ms": 704.0,   # 2 x (edge 108 + U 32 + flux 60) + 136 + 168
 }
 METRIC = "cell-updates/s (fp64 MUSCL-RK2, 13M cells) and achieved HBM GB/s vs ~8 TB/s"
+PAPER_CONTEXT = {   # whole-simulation wall times, step counts not stated -> context only
+    "muscl": "paper Table 5 (PAPER.md:483), 13 M-triangle Mille Iles mesh, MUSCL, 2 ghost layers, high overlap: "
+             "326.38 s on 8 P100 ... 90.08 s on 32 P100 (whole simulation; number of steps not stated)",
+    "muscl_ms": "paper Table 5 (PAPER.md:483), MUSCL (the multislope scheme is the paper's own), 2 layers, high overlap: "
+                "326.38 s on 8 P100 ... 90.08 s on 32 P100 (whole simulation; number of steps not stated)",
+    "hllc": "paper Table 5 (PAPER.md:481), HLLC, 1 ghost layer, high overlap: 205.26 s on 8 P100 ... 60.63 s on 32 P100 "
+            "(whole simulation; number of steps not stated)",
+    "waf": "paper Table 5 (PAPER.md:484), WAF, 2 ghost layers, high overlap: 329.56 s on 8 P100 ... 90.82 s on 32 P100 "
+           "(whole simulation; number of steps not stated)",
+}
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
 
 
@@ -298,7 +308,8 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
                        "parallelism": "zones over %d ranks (%d zones, %d ghost layers), halo transport %s, "
                                       "schedule %s, all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport,
                                                                               S.schedule),
-                       "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo},
+                       "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo,
+                       "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": None,
             "gpu_launches": int(launches), "clocks": clocks,
         }
@@ -418,7 +429,7 @@ def main():
                        if nt > 2_000_000 else "working set may fit L2 at this size",
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
                        "zones": args.zones, "ghost_layers": args.layers if args.zones else 0,
-                       "renumber": args.renumber},
+                       "renumber": args.renumber, "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
             "gpu_launches": l1["kernel_launches"] - l0["kernel_launches"], "clocks": clocks,
         }
