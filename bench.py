@@ -293,9 +293,10 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
     torch.cuda.synchronize()
     e2e_s = swdist.reduce_max(time.perf_counter() - t0)
     e2e = {"value": nt * e2e_steps / e2e_s, "unit": "cell-updates/s", "steps": e2e_steps,
-           "h2d_bytes_per_step": 3 * 8 * nt * world, "d2h_bytes_per_step": 3 * 8 * nt * world,
+           "h2d_bytes_per_step": 2 * 3 * 8 * nt * world, "d2h_bytes_per_step": 3 * 8 * nt * world,
            "what": "per step and rank: swe_set_state(full state, pinned host) + one distributed step + "
-                   "swe_get_state(pinned host; the rank's own cells are filled)"}
+                   "swe_get_state(pinned host; the rank's own cells are filled, which stages the caller's "
+                   "arrays through the device: a second host-to-device copy)"}
     S.close()
     if rank == 0:
         line = {
