@@ -184,6 +184,20 @@ def flooded(cfg, level):
     return out
 
 
+def delaunay_case(n=3000, lx=200.0, ly=120.0, seed=5, level=3.0, dam=True):
+    """An unstructured (Delaunay) mesh over a bumpy bed with dry bump tops: lake at rest at `level`
+    (dam=False) or the same with the left third raised by 2 m (a dam break running over the bumps
+    and around the dry tops).  Walls all round, Manning 0.03."""
+    from .meshes import delaunay_mesh
+    x, y, tri = delaunay_mesh(n, lx, ly, seed)
+    zb = gaussian_bumps(x, y, seed, 10, max(lx, ly), 2.0, 6.0, 8.0, 25.0) + value_noise(x, y, seed, 3, 0.3, 40.0)
+    zc = _cell_bed(zb, tri)
+    cx, _ = _centroids(x, y, tri)
+    eta = np.where((cx < lx / 3.0) & dam, level + 2.0, level)
+    h = np.maximum(0.0, eta - zc)
+    return _base("delaunay", x, y, zb, tri, h, [("muscl", 0.45, 100)], manning=np.full(tri.shape[0], 0.03))
+
+
 def channel_flow_case(nx=100, ny=5, lx=100.0, ly=5.0, jitter=0.1, seed=4, discharge=10.0, level=2.0,
                       manning=0.0, h_init=None, u_init=0.0):
     """Straight flat channel with the two open boundaries of configs[3]: imposed discharge Q on the

@@ -45,6 +45,47 @@ def grid_mesh(nx, ny, lx, ly, jitter=0.0, seed=0, permute=False):
     return x, y, np.ascontiguousarray(tri)
 
 
+def delaunay_mesh(n, lx, ly, seed=0):
+    """A genuinely unstructured triangulation of [0,lx]x[0,ly]: n seeded random interior points
+    (rejected if closer than 0.45 of the mean spacing to an earlier one) plus equispaced boundary
+    points, Delaunay-triangulated (scipy).  Vertex valence, triangle shape, winding and order are
+    whatever the triangulator returns (every third triangle is then turned clockwise); needle
+    triangles along the boundary are dropped."""
+    from scipy.spatial import Delaunay, cKDTree
+    rng = np.random.default_rng(seed)
+    spacing = np.sqrt(lx * ly / n)
+    nbx, nby = max(2, int(round(lx / spacing))), max(2, int(round(ly / spacing)))
+    bx = np.linspace(0.0, lx, nbx + 1)
+    by = np.linspace(0.0, ly, nby + 1)
+    border = np.concatenate([np.stack([bx, np.zeros_like(bx)], 1), np.stack([bx, np.full_like(bx, ly)], 1),
+                             np.stack([np.zeros_like(by[1:-1]), by[1:-1]], 1),
+                             np.stack([np.full_like(by[1:-1], lx), by[1:-1]], 1)])
+    cand = rng.uniform([0.3 * spacing, 0.3 * spacing], [lx - 0.3 * spacing, ly - 0.3 * spacing], (3 * n, 2))
+    pts = list(border)
+    tree_pts = np.array(pts)
+    keep = []
+    for start in range(0, cand.shape[0], 256):                     # thinning in blocks
+        block = cand[start:start + 256]
+        tree = cKDTree(np.concatenate([tree_pts, np.array(keep).reshape(-1, 2)]))
+        d, _ = tree.query(block)
+        ok = block[d > 0.45 * spacing]
+        if ok.shape[0]:
+            sub = cKDTree(ok)
+            pairs = sub.query_pairs(0.45 * spacing)
+            drop = {j for _, j in pairs}
+            keep.extend(ok[[i for i in range(ok.shape[0]) if i not in drop]])
+        if len(keep) >= n:
+            break
+    p = np.concatenate([border, np.array(keep[:n]).reshape(-1, 2)])
+    tri = Delaunay(p).simplices.astype(np.int32)
+    a = p[tri[:, 1]] - p[tri[:, 0]]
+    b = p[tri[:, 2]] - p[tri[:, 0]]
+    area = 0.5 * np.abs(a[:, 0] * b[:, 1] - a[:, 1] * b[:, 0])
+    tri = tri[area > 1e-3 * spacing * spacing]                      # collinear boundary points give slivers
+    tri[::3] = tri[::3, ::-1]                                       # every third triangle clockwise
+    return np.ascontiguousarray(p[:, 0]), np.ascontiguousarray(p[:, 1]), np.ascontiguousarray(tri)
+
+
 def boundary_edges(tri):
     """Vertex pairs (nb,2) of edges that belong to exactly one triangle (used only to attach
     boundary tags; the libraries find boundary edges themselves)."""

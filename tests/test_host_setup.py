@@ -9,7 +9,7 @@ import pytest
 
 import paper_2307_16758_b200 as sw
 from oracle import pyoracle as po
-from swe_inputs import config0, config1, config3, lake_case
+from swe_inputs import config0, config1, config3, lake_case, delaunay_case
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -41,10 +41,11 @@ def _cases():
         "c1": config1(n=24),
         "lake": lake_case(n=20),
         "river": config3(length=1600.0, half_width=400.0, w2=20.0, n4=3, n8=2),
+        "delaunay": delaunay_case(n=1500),          # genuinely unstructured, mixed windings
     }
 
 
-@pytest.mark.parametrize("name", ["c0", "c1", "lake", "river"])
+@pytest.mark.parametrize("name", ["c0", "c1", "lake", "river", "delaunay"])
 @pytest.mark.parametrize("renum", [sw.SWE_RENUM_NONE, sw.SWE_RENUM_HILBERT, sw.SWE_RENUM_RCM])
 def test_host_mesh_matches_oracle_geometry(name, renum):
     cfg = _cases()[name]
@@ -147,7 +148,8 @@ def test_hilbert_order_is_local():
         sw.swe_host_mesh_free(h0)
 
 
-@pytest.mark.parametrize("name,nz,nl", [("c1", 4, 2), ("c1", 8, 1), ("river", 4, 3), ("lake", 2, 2)])
+@pytest.mark.parametrize("name,nz,nl", [("c1", 4, 2), ("c1", 8, 1), ("river", 4, 3), ("lake", 2, 2),
+                                        ("delaunay", 8, 2), ("delaunay", 4, 3)])
 def test_zone_builder_matches_oracle(name, nz, nl):
     cfg = _cases()[name]
     o = po.Oracle.from_config(cfg)
