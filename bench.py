@@ -59,6 +59,10 @@ def build_workload(name):
     if name == "c3w":
         from swe_inputs import flooded
         return flooded(config3(), 18.0), "configs[3] mesh and bed, flooded to a flat surface at 18 m: no dry cell"
+    if name == "dl":
+        from swe_inputs import delaunay_case
+        return (delaunay_case(n=3_000_000, lx=20000.0, ly=12000.0, seed=5, dam=True),
+                "Delaunay triangulation of 3 M jittered points (~6 M triangles, mixed windings), dam break over bumps with dry tops, seed 5")
     if name == "c3s":
         return config3(length=6000.0), "configs[3] generator on a 6 km reach (~1.3 M triangles), seed 3"
     if name == "c3t":
@@ -324,7 +328,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3p", "c3w", "c3s", "c3t", "c1", "c2"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3p", "c3w", "dl", "c3s", "c3t", "c1", "c2"])
     ap.add_argument("--scheme", default="muscl", choices=["muscl", "hllc", "waf", "muscl_ms"])
     ap.add_argument("--zones", type=int, default=0)
     ap.add_argument("--layers", type=int, default=2)

@@ -190,7 +190,8 @@ def delaunay_case(n=3000, lx=200.0, ly=120.0, seed=5, level=3.0, dam=True):
     and around the dry tops).  Walls all round, Manning 0.03."""
     from .meshes import delaunay_mesh
     x, y, tri = delaunay_mesh(n, lx, ly, seed)
-    zb = gaussian_bumps(x, y, seed, 10, max(lx, ly), 2.0, 6.0, 8.0, 25.0) + value_noise(x, y, seed, 3, 0.3, 40.0)
+    sc = lx / 200.0                                   # bump widths and noise wavelength follow the domain
+    zb = gaussian_bumps(x, y, seed, 10, max(lx, ly), 2.0, 6.0, 8.0 * sc, 25.0 * sc) + value_noise(x, y, seed, 3, 0.3, 40.0 * sc)
     zc = _cell_bed(zb, tri)
     cx, _ = _centroids(x, y, tri)
     eta = np.where((cx < lx / 3.0) & dam, level + 2.0, level)

@@ -60,6 +60,20 @@ def delaunay_mesh(n, lx, ly, seed=0):
     border = np.concatenate([np.stack([bx, np.zeros_like(bx)], 1), np.stack([bx, np.full_like(bx, ly)], 1),
                              np.stack([np.zeros_like(by[1:-1]), by[1:-1]], 1),
                              np.stack([np.full_like(by[1:-1], lx), by[1:-1]], 1)])
+    if n > 50000:
+        # large meshes: one point per lattice site, displaced by up to 0.45 of the spacing (the
+        # Poisson-disc thinning below is a Python loop); the connectivity is still the triangulator's
+        gx, gy = np.meshgrid(bx[1:-1], by[1:-1], indexing="xy")
+        inner = np.stack([gx.ravel(), gy.ravel()], 1)
+        inner += rng.uniform(-0.45, 0.45, inner.shape) * [lx / nbx, ly / nby]
+        p = np.concatenate([border, inner])
+        tri = Delaunay(p).simplices.astype(np.int32)
+        a = p[tri[:, 1]] - p[tri[:, 0]]
+        b = p[tri[:, 2]] - p[tri[:, 0]]
+        area = 0.5 * np.abs(a[:, 0] * b[:, 1] - a[:, 1] * b[:, 0])
+        tri = tri[area > 1e-3 * spacing * spacing]
+        tri[::3] = tri[::3, ::-1]
+        return np.ascontiguousarray(p[:, 0]), np.ascontiguousarray(p[:, 1]), np.ascontiguousarray(tri)
     cand = rng.uniform([0.3 * spacing, 0.3 * spacing], [lx - 0.3 * spacing, ly - 0.3 * spacing], (3 * n, 2))
     pts = list(border)
     tree_pts = np.array(pts)
