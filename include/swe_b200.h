@@ -219,7 +219,8 @@ int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_o
  * bandwidth-bound claim is checked against.  Synchronises. */
 int swe_fp64_peak(swe_ctx* ctx, double* tflops_out);
 /* per-kernel timing: runs `reps` launches of one kernel of the hot path on the current state
- * between two events; which: 0 dt_reduce, 1 grad_limit, 2 edge_flux(scheme), 3 cell_update (Euler
+ * between two events; which: 0 dt_reduce, 1 grad_limit (scheme SWE_MUSCL_MS: the multislope side
+ * records, k_ms_slopes), 2 edge_flux(scheme), 3 cell_update (Euler
  * stage), 4 cell_update (Heun combine), 5 pack, 6 unpack.  The state is left unchanged (updates
  * write to the stage buffer). */
 int swe_kernel_timed(swe_ctx* ctx, int which, int scheme, int reps, float* ms_out);
@@ -227,7 +228,8 @@ int swe_kernel_timed(swe_ctx* ctx, int which, int scheme, int reps, float* ms_ou
 /* per-kernel timing inside swe_step: with profiling on, every kernel launch of swe_step is
  * bracketed by two CUDA events on the context's stream; swe_get_profile synchronises and returns
  * accumulated milliseconds and launch counts per kind (7 each):
- * 0 dt_reduce, 1 grad_limit, 2 edge_flux, 3 cell_update, 4 pack, 5 unpack, 6 dt_finalize. */
+ * 0 dt_reduce, 1 grad_limit (or the multislope side records), 2 edge_flux, 3 cell_update (both the
+ * full and the send-list launches), 4 pack (and the peer-memory push), 5 unpack, 6 dt_finalize. */
 int swe_set_profile(swe_ctx* ctx, int on);
 int swe_get_profile(swe_ctx* ctx, double* ms, int64_t* count);
 
