@@ -607,8 +607,9 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         Z.rrecv_off[p + 1] = (int64_t)Z.rrecv_idx.size();
     }
     // ---- cells on any send list (remote or resident), ascending: the overlap schedule updates them
-    // first; they carry -1 in c2e.w (owned cells otherwise carry 0) ----
-    if (nranks > 1) {
+    // first; they carry -1 in c2e.w (owned cells otherwise carry 0).  Built for one rank too: the
+    // links between resident zones are served by the same exchange ----
+    {
         Z.send_cells = Z.rsend_idx;
         Z.send_cells.insert(Z.send_cells.end(), Z.send_idx.begin(), Z.send_idx.end());
         std::sort(Z.send_cells.begin(), Z.send_cells.end());

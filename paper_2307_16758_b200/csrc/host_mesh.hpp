@@ -69,7 +69,7 @@ struct ZoneSet {
     std::vector<int32_t> rsend_peer;         // and the peer rank (for the one-kernel push over peer memory)
     std::vector<int32_t> rrecv_idx;          // resident ghost cells filled from remote owners
     std::vector<int64_t> rsend_off, rrecv_off;   // nranks + 1 each
-    std::vector<int32_t> send_cells;         // nranks > 1: distinct resident cells on any send list, ascending
+    std::vector<int32_t> send_cells;         // distinct resident cells on any send list (remote or resident), ascending
 };
 
 struct HostMesh {

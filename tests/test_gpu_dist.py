@@ -281,3 +281,59 @@ def test_bench_line_of_the_distributed_arm(extra):
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["achieved"] > 0 and r["peak"] > 0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0 and d["cpu_baseline"] is None
+
+
+def _nccl_worker(port, schedule, transport, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK="0", LOCAL_RANK="0", WORLD_SIZE="1", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    os.environ.pop("SWE_DIST_GLOO", None)
+    try:
+        import torch.distributed as dist
+        from paper_2307_16758_b200 import dist as d
+        torch.cuda.set_device(0)
+        dist.init_process_group(backend="nccl", rank=0, world_size=1)
+        cfg = _river()
+        S = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport, schedule=schedule)
+        assert not S.comm.staged_host                      # the NCCL code path, not the host-staged one
+        S.step(8, 0.45, "muscl")
+        S.step(7, 0.9, "hllc")
+        S.step(5, 0.45, "waf")
+        t = S.time()
+        st = S.get_state()
+        S.set_state(*[torch.from_numpy(x.copy()) for x in st])
+        S.step(3, 0.45, "muscl_ms")
+        st2 = S.get_state()
+        S.close()
+        a = sw.create_from_config(cfg)
+        sw.swe_step(a, 8, 0.45, "muscl"); sw.swe_step(a, 7, 0.9, "hllc")
+        ta = sw.swe_step(a, 5, 0.45, "waf")
+        ref = sw.swe_get_state(a)
+        sw.swe_step(a, 3, 0.45, "muscl_ms")
+        ref2 = sw.swe_get_state(a)
+        sw.swe_mesh_destroy(a)
+        checks = [ta == t] + [bool(np.array_equal(x, y)) for x, y in zip(ref, st)] + \
+                 [bool(np.array_equal(x, y)) for x, y in zip(ref2, st2)]
+        dist.destroy_process_group()
+        q.put((all(checks), "" if all(checks) else "time / h hu hv after the first run / after set_state: %s (t %r vs %r)"
+               % (checks, t, ta)))
+    except Exception as e:
+        import traceback
+        q.put((False, traceback.format_exc() + str(e)))
+
+
+@pytest.mark.parametrize("schedule,transport", [("overlap", "p2p"), ("plain", "staged"), ("overlap", "staged")])
+def test_dist_solver_over_nccl_single_rank(schedule, transport):
+    """The NCCL code path of dist.py (asynchronous all-reduces on NCCL's stream and work.wait(),
+    device tensors in every collective) with the one rank one GPU allows: 4 resident zones."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_nccl_worker, args=(29600 + os.getpid() % 90, schedule, transport, q))
+    p.start()
+    try:
+        ok, msg = q.get(timeout=600)
+        p.join(120)
+    finally:
+        if p.is_alive():
+            p.kill()
+    assert msg == "", msg
+    assert ok
