@@ -337,3 +337,56 @@ def test_dist_solver_over_nccl_single_rank(schedule, transport):
             p.kill()
     assert msg == "", msg
     assert ok
+
+
+def _mixed_worker(rank, world, port, transport, schedule, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port), SWE_DIST_GLOO="1")
+    seq = [("muscl", 0.45, 6), ("hllc", 0.9, 5), ("waf", 0.45, 4), ("muscl_ms", 0.45, 3), ("hllc", 0.9, 1), ("muscl", 0.45, 2)]
+    try:
+        from paper_2307_16758_b200 import dist as d
+        d.init_from_env()
+        cfg = _river()
+        S = d.DistSolver(cfg, nzones=8, nlayers=2, transport=transport, schedule=schedule)
+        for scheme, cfl, n in seq:
+            S.step(n, cfl, scheme)
+        t = S.time()
+        st = S.get_state()
+        S.close()
+        out = None
+        if rank == 0:
+            a = sw.create_from_config(cfg)
+            for scheme, cfl, n in seq:
+                ta = sw.swe_step(a, n, cfl, scheme)
+            ref = sw.swe_get_state(a)
+            sw.swe_mesh_destroy(a)
+            out = bool(ta == t and all(np.array_equal(x, y) for x, y in zip(ref, st)))
+        d.finalize()
+        q.put((rank, out, ""))
+    except Exception as e:
+        import traceback
+        q.put((rank, False, traceback.format_exc() + str(e)))
+
+
+@pytest.mark.parametrize("transport,schedule", [("p2p", "overlap"), ("staged", "overlap"), ("p2p", "plain")])
+def test_two_processes_scheme_changes_between_calls(transport, schedule):
+    """The overlap schedule leaves an exchange and an all-reduce in flight between calls: changing the
+    scheme from call to call (Heun <-> Euler, WAF's early dt) must not disturb them.  8 zones on 2
+    ranks: remote and resident links together."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 90
+    ps = [ctx.Process(target=_mixed_worker, args=(r, 2, port, transport, schedule, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    try:
+        res = sorted(q.get(timeout=600) for _ in ps)
+        for p in ps:
+            p.join(120)
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.kill()
+    assert all(r[2] == "" for r in res), [r[2] for r in res]
+    assert res[0][1] is True
