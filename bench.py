@@ -335,6 +335,8 @@ def main():
     ap.add_argument("--renumber", default="hilbert", choices=["hilbert", "rcm", "none"])
     ap.add_argument("--transport", default="p2p", choices=["p2p", "staged"])
     ap.add_argument("--schedule", default="overlap", choices=["overlap", "plain"])
+    ap.add_argument("--force-dist", action="store_true",
+                    help="run the distributed arm (DistSolver, zones over ranks) even with a single rank")
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -357,7 +359,12 @@ def main():
 
     cfg, desc = build_workload(args.workload)
     cfl = 0.9 if args.scheme == "hllc" else 0.45
-    if world > 1 and not args.replicas:
+    if args.force_dist and world == 1:
+        import torch.distributed as tdist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+        tdist.init_process_group(backend="gloo" if os.environ.get("SWE_DIST_GLOO") else "nccl", rank=0, world_size=1)
+    if (world > 1 and not args.replicas) or args.force_dist:
         return run_dist(args, rank, world, local, cfg, desc, cfl)
     ctx = sw.create_from_config(cfg, {"hilbert": sw.SWE_RENUM_HILBERT, "rcm": sw.SWE_RENUM_RCM,
                                       "none": sw.SWE_RENUM_NONE}[args.renumber])
