@@ -106,8 +106,16 @@ int swe_set_graphs(swe_ctx* ctx, int on);
  *            recursive coordinate bisection (nzones must then be a power of two)
  *   nlayers: ghost layers per zone, 1..3 (edge adjacency)
  * Each zone gets its own copy of its owned + ghost cells; per (zone, source zone) one send list
- * (indices into the source zone) and one contiguous receive range.  nzones == 0 removes zones. */
+ * (indices into the source zone) and one contiguous receive range.  nzones == 0 removes zones.
+ * The ghost layers and their numbering (sections 3.2-3.3)
+ * are generated on the device: the layers of all zones grow together as bit masks over the edge
+ * adjacency, one launch per layer, and a radix sort of (zone, source zone, layer, cell) keys gives
+ * the contiguous receive ranges (csrc/swe_zone_kernels.cuh). */
 int swe_zones_create(swe_ctx* ctx, int nzones, int nlayers, const int32_t* zone_of_cell);
+/* wall-clock milliseconds of the last swe_zones_create / swe_zones_create_dist (host pointers,
+ * any may be NULL): the device ghost-layer generation alone; the whole zone build up to the
+ * concatenated host arrays; the whole call including the upload.  SWE_ERR_STATE without zones. */
+int swe_zone_setup_ms(const swe_ctx* ctx, double* ghost_layers_ms, double* build_ms, double* total_ms);
 /* pack: send buffer[k] = U[send_idx[k]] for every link whose SOURCE is `zone` (-1 = all zones);
  * unpack: copy the buffers into the contiguous ghost ranges of `zone` (-1 = all). */
 int swe_pack_ghosts(swe_ctx* ctx, int zone);

@@ -43,6 +43,7 @@ SIGNATURES = {
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_unpack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_zone_stats": (C.c_int, [_vp, _i64p, _i64p, _i64p]),
+    "swe_zone_setup_ms": (C.c_int, [_vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "swe_zone_describe": (C.c_int, [_vp, C.c_int, _i64p, _i64p, _i64p]),
     "swe_zone_cells": (C.c_int, [_vp, C.c_int, _vp, _vp]),
     "swe_zone_links": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
@@ -228,6 +229,13 @@ def swe_zone_stats(ctx):
     a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
     _check(lib().swe_zone_stats(ctx, C.byref(a), C.byref(b), C.byref(c)))
     return {"send_cells_total": a.value, "bytes_per_exchange": b.value, "ghost_cells_total": c.value}
+
+
+def swe_zone_setup_ms(ctx):
+    """wall-clock ms of the last swe_zones_create: device ghost layers, zone build, whole call."""
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().swe_zone_setup_ms(ctx, C.byref(a), C.byref(b), C.byref(c)))
+    return {"ghost_layers_ms": a.value, "build_ms": b.value, "total_ms": c.value}
 
 
 def swe_zone_describe_counts(ctx, zone):

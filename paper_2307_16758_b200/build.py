@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswe_b200.so")
 SRCS = ["swe_api.cu", "host_mesh.cpp", "host_inspect.cpp"]
-DEPS = SRCS + ["swe_kernels.cuh", "host_mesh.hpp", os.path.join("..", "..", "include", "swe_b200.h")]
+DEPS = SRCS + ["swe_kernels.cuh", "swe_zone_kernels.cuh", "host_mesh.hpp", os.path.join("..", "..", "include", "swe_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 EXTRA = os.environ.get("SWE_NVCC_EXTRA", "").split()   # e.g. -DSWE_FLUX_MINB=4 for tuning sweeps

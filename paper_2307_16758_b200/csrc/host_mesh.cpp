@@ -389,7 +389,8 @@ void rcb_split(const HostMesh& H, std::vector<int32_t>& ids, int z0, int nz, std
 }  // namespace
 
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32_t* zone_of_cell_user,
-                 std::string& err, int nranks, int rank, const int32_t* zone_begin) {
+                 std::string& err, int nranks, int rank, const int32_t* zone_begin,
+                 const GhostFinder& ghost_finder) {
     const MeshArrays& G = H.m;
     const int64_t nc = G.nc;
     Z = ZoneSet();
@@ -427,32 +428,48 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         owned_pos[i] = (int32_t)zd.cells.size();
         zd.cells.push_back((int32_t)i);
     }
-    // A.12.2 ghost layers by breadth-first search over edge adjacency; A.12.3 numbering
-    std::vector<int32_t> mark(nc, -1);
+    // A.12.2 ghost layers = breadth-first distance over the edge adjacency; A.12.3 numbering.
+    // From the device generator (sorted keys of all zones) when the library runs, by the host
+    // search below when the set-up is inspected without a GPU.
+    std::vector<uint64_t> keys;
+    if (ghost_finder) {
+        if ((int64_t)nz * nz > (int64_t)1 << 29) { err = "too many zones"; return false; }
+        if (!ghost_finder(Z.zone_of, nz, nlayers, keys, err)) return false;
+    }
+    size_t kpos = 0;
+    std::vector<int32_t> mark(ghost_finder ? 0 : nc, -1);
     struct Gh { int32_t cell, layer, src; };
     for (int zi = 0; zi < nz; ++zi) {
         ZoneDesc& zd = Z.z[zi];
         zd.nowned = (int64_t)zd.cells.size();
         zd.layer.assign(zd.cells.size(), 0);
-        for (int32_t i : zd.cells) mark[i] = zi;
-        std::vector<int32_t> frontier = zd.cells, next;
         std::vector<Gh> ghosts;
-        for (int l = 1; l <= nlayers; ++l) {
-            next.clear();
-            for (int32_t i : frontier)
-                for (int k = 0; k < 3; ++k) {
-                    int32_t nbq = G.c2c[4 * (int64_t)i + k];
-                    if (nbq >= 0 && mark[nbq] != zi) {
-                        mark[nbq] = zi; next.push_back(nbq);
-                        ghosts.push_back(Gh{nbq, l, Z.zone_of[nbq]});
+        if (ghost_finder) {
+            for (; kpos < keys.size(); ++kpos) {
+                const uint64_t b = keys[kpos] >> 32;
+                if ((int64_t)((b >> 2) / (uint64_t)nz) != zi) break;
+                ghosts.push_back(Gh{(int32_t)(keys[kpos] & 0xffffffffu), (int32_t)(b & 3), (int32_t)((b >> 2) % (uint64_t)nz)});
+            }
+        } else {
+            for (int32_t i : zd.cells) mark[i] = zi;
+            std::vector<int32_t> frontier = zd.cells, next;
+            for (int l = 1; l <= nlayers; ++l) {
+                next.clear();
+                for (int32_t i : frontier)
+                    for (int k = 0; k < 3; ++k) {
+                        int32_t nbq = G.c2c[4 * (int64_t)i + k];
+                        if (nbq >= 0 && mark[nbq] != zi) {
+                            mark[nbq] = zi; next.push_back(nbq);
+                            ghosts.push_back(Gh{nbq, l, Z.zone_of[nbq]});
+                        }
                     }
-                }
-            frontier.swap(next);
+                frontier.swap(next);
+            }
+            std::sort(ghosts.begin(), ghosts.end(), [](const Gh& a, const Gh& b) {
+                if (a.src != b.src) return a.src < b.src;
+                if (a.layer != b.layer) return a.layer < b.layer;
+                return a.cell < b.cell; });
         }
-        std::sort(ghosts.begin(), ghosts.end(), [](const Gh& a, const Gh& b) {
-            if (a.src != b.src) return a.src < b.src;
-            if (a.layer != b.layer) return a.layer < b.layer;
-            return a.cell < b.cell; });
         for (const Gh& gq : ghosts) {
             if (zd.links.empty() || zd.links.back().src != gq.src) {
                 ZoneLink lk; lk.src = gq.src; lk.start = (int32_t)zd.cells.size(); lk.count = 0;
@@ -465,6 +482,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             zd.layer.push_back(gq.layer);
         }
     }
+    if (kpos != keys.size()) { err = "ghost keys are not sorted by zone"; return false; }
     // offset of every zone in the concatenated mesh of the rank that holds it
     std::vector<int64_t> owner_off(nz, 0), rank_cells(nranks, 0);
     for (int zi = 0; zi < nz; ++zi) {

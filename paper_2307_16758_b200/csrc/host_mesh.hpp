@@ -4,6 +4,7 @@
 // geometry is the literal IEEE evaluation of the formulas of A.1.
 #pragma once
 #include <cstdint>
+#include <functional>
 #include <string>
 #include <vector>
 
@@ -89,8 +90,15 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
 
 // Builds the zone decomposition and the concatenated zoned mesh.  zone_of_cell_user may be null
 // (recursive coordinate bisection).  Returns false and sets err on invalid arguments.
+// ghost_finder (row f4, may be empty): returns the ghost entries of ALL zones as sorted 64-bit keys
+//   ((z * nzones + src) * 4 + layer) << 32 | cell      (cell, src = zone_of[cell]: un-zoned device ids)
+// i.e. in the order of A.12.3 (zone, source zone, layer, cell).  The library passes the device
+// generator of swe_zone_kernels.cuh; without one the layers come from the host breadth-first
+// search below (the host-inspection entry points, which must run without a GPU).
+using GhostFinder = std::function<bool(const std::vector<int32_t>& zone_of, int nzones, int nlayers,
+                                       std::vector<uint64_t>& keys, std::string& err)>;
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nzones, int nlayers,
                  const int32_t* zone_of_cell_user, std::string& err, int nranks = 1, int rank = 0,
-                 const int32_t* zone_begin = nullptr);
+                 const int32_t* zone_begin = nullptr, const GhostFinder& ghost_finder = GhostFinder());
 
 }  // namespace swe

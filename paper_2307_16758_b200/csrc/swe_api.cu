@@ -3,7 +3,9 @@
 #include "../../include/swe_b200.h"
 #include "host_mesh.hpp"
 #include "swe_kernels.cuh"
+#include "swe_zone_kernels.cuh"
 
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -93,6 +95,7 @@ struct swe_ctx {
     double4** d_peerB = nullptr;
     std::vector<void*> peerA, peerB;   // host copies; [rank] = this context's own buffers
     std::vector<char> peer_ipc;        // 1: opened with cudaIpcOpenMemHandle (closed in free_zones)
+    double zone_ms[3] = {0, 0, 0};     // last swe_zones_create: device ghost layers, + host zone build, + upload (cumulative)
     int* d_send_cells = nullptr;       // distinct cells on a send list (overlap schedule updates them first)
     int64_t nsendcells = 0;
     // staging for host pointers
@@ -866,6 +869,74 @@ int swe_get_stats(const swe_ctx* c, int64_t* steps, int64_t* kernel_launches, in
 }
 
 // ---- zones ----
+// Row f4: the ghost layers of all zones on the device (swe_zone_kernels.cuh).  zone_of: per cell of
+// the un-zoned mesh, device numbering.  Returns the sorted keys build_zones consumes.
+static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, int nz, int nlayers,
+                              std::vector<uint64_t>& keys, std::string& err) {
+    const int nc = (int)c->g.nc;
+    const int W = (nz + 63) / 64;
+    const size_t words = (size_t)W * nc;
+    int* d_zone = nullptr;
+    unsigned long long *d_reach[2] = {nullptr, nullptr}, *d_fresh[3] = {nullptr, nullptr, nullptr};
+    unsigned long long *d_count = nullptr, *d_keys[2] = {nullptr, nullptr};
+    unsigned int* d_hist = nullptr;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
+    auto cleanup = [&] {
+        cudaFree(d_zone); cudaFree(d_reach[0]); cudaFree(d_reach[1]);
+        for (auto p : d_fresh) cudaFree(p);
+        cudaFree(d_count); cudaFree(d_keys[0]); cudaFree(d_keys[1]); cudaFree(d_hist);
+    };
+    keys.clear();
+    const int grid = grid_for(nc, c->grid_light);
+    unsigned long long total = 0;
+    if (ok(cudaMalloc((void**)&d_zone, (size_t)nc * sizeof(int))) &&
+        ok(cudaMalloc((void**)&d_reach[0], words * 8)) && ok(cudaMalloc((void**)&d_reach[1], words * 8)) &&
+        ok(cudaMalloc((void**)&d_count, 2 * sizeof(unsigned long long)))) {
+        for (int l = 0; l < nlayers; ++l) ok(cudaMalloc((void**)&d_fresh[l], words * 8));
+    }
+    if (e == cudaSuccess) {
+        ok(cudaMemcpyAsync(d_zone, zone_of.data(), (size_t)nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        ok(cudaMemsetAsync(d_count, 0, 2 * sizeof(unsigned long long), c->stream));
+        k_gl_seed<<<grid, 256, 0, c->stream>>>(d_zone, d_reach[0], nc, W);
+        for (int l = 0; l < nlayers; ++l)
+            k_gl_grow<<<grid, 256, 0, c->stream>>>(c->g.dm.c2c, d_reach[l & 1], d_reach[(l + 1) & 1], d_fresh[l], nc, W, d_count);
+        c->launches += 1 + nlayers;
+        ok(cudaGetLastError());
+        ok(cudaMemcpyAsync(&total, d_count, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
+        ok(cudaStreamSynchronize(c->stream));
+    }
+    if (e == cudaSuccess && total > 0) {
+        if (total > (unsigned long long)INT32_MAX) { cleanup(); err = "too many ghost cells"; return false; }
+        const long long n = (long long)total;
+        const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
+        if (ok(cudaMalloc((void**)&d_keys[0], (size_t)n * 8)) && ok(cudaMalloc((void**)&d_keys[1], (size_t)n * 8)) &&
+            ok(cudaMalloc((void**)&d_hist, (size_t)256 * nblk * sizeof(unsigned int)))) {
+            for (int l = 0; l < nlayers; ++l)
+                k_gl_emit<<<grid, 256, 0, c->stream>>>(d_fresh[l], d_zone, l + 1, nz, nc, W, d_keys[0], d_count + 1);
+            // significant key bits: 32 (cell) + those of the largest bucket (nz * nz * 4 - 1)
+            int bits = 32;
+            for (unsigned long long top = (unsigned long long)nz * nz * 4ull - 1ull; top; top >>= 1) ++bits;
+            int cur = 0;
+            for (int shift = 0; shift < bits; shift += 8) {
+                k_rs_hist<<<nblk, RS_THREADS, 0, c->stream>>>(d_keys[cur], n, shift, d_hist, nblk);
+                k_rs_scan<<<1, 1024, 0, c->stream>>>(d_hist, (long long)256 * nblk);
+                k_rs_scatter<<<nblk, RS_THREADS, 0, c->stream>>>(d_keys[cur], d_keys[cur ^ 1], n, shift, d_hist, nblk);
+                cur ^= 1;
+                c->launches += 3;
+            }
+            c->launches += nlayers;
+            ok(cudaGetLastError());
+            keys.resize((size_t)n);
+            ok(cudaMemcpyAsync(keys.data(), d_keys[cur], (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream));
+            ok(cudaStreamSynchronize(c->stream));
+        }
+    }
+    cleanup();
+    if (e != cudaSuccess) { cudaGetLastError(); err = std::string("device ghost-layer generation: ") + cudaGetErrorString(e); return false; }
+    return true;
+}
+
 static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell, int nranks,
                              int rank, const int32_t* zone_begin) {
     if (check_ctx(c)) return SWE_ERR_ARG;
@@ -884,9 +955,19 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     }
     std::string err;
     bool ok = false;
-    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err, nranks, rank, zone_begin); }
+    const auto t0 = std::chrono::steady_clock::now();
+    double ghost_ms = 0.0;
+    GhostFinder finder = [&](const std::vector<int32_t>& zone_of, int nz, int nl, std::vector<uint64_t>& keys, std::string& er) {
+        const auto g0 = std::chrono::steady_clock::now();
+        const bool r = device_ghost_keys(c, zone_of, nz, nl, keys, er);
+        ghost_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - g0).count();
+        return r;
+    };
+    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err, nranks, rank, zone_begin, finder); }
     catch (const std::bad_alloc&) { c->Z = ZoneSet(); return fail(SWE_ERR_NOMEM, "out of host memory in zone set-up"); }
     if (!ok) { c->Z = ZoneSet(); return fail(SWE_ERR_ARG, err); }
+    c->zone_ms[0] = ghost_ms;
+    c->zone_ms[1] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     rc = upload_store(c, c->z, c->Z.mesh);
     if (rc) { free_zones(c); return rc; }
     c->z.dm.glayer = (nlayers >= 2) ? 1 : 0;
@@ -936,6 +1017,7 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     CU(cudaStreamSynchronize(c->stream));
     // the host copies of the big zoned arrays are no longer needed
     c->Z.mesh = MeshArrays();
+    c->zone_ms[2] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     return SWE_OK;
 }
 
@@ -1168,6 +1250,14 @@ int swe_zone_stats(const swe_ctx* c, int64_t* send_cells_total, int64_t* bytes_p
     if (send_cells_total) *send_cells_total = c->nsend;
     if (bytes_per_exchange) *bytes_per_exchange = c->nsend * 24;
     if (ghost_cells_total) *ghost_cells_total = gh;
+    return SWE_OK;
+}
+int swe_zone_setup_ms(const swe_ctx* c, double* ghost_layers_ms, double* build_ms, double* total_ms) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (ghost_layers_ms) *ghost_layers_ms = c->zone_ms[0];
+    if (build_ms) *build_ms = c->zone_ms[1];
+    if (total_ms) *total_ms = c->zone_ms[2];
     return SWE_OK;
 }
 int swe_zone_describe(const swe_ctx* c, int zone, int64_t* nowned, int64_t* nghost, int64_t* nlinks) {
