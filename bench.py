@@ -417,6 +417,8 @@ def main():
            "h2d_bytes_per_step": 3 * 8 * nt, "d2h_bytes_per_step": 3 * 8 * nt,
            "what": "per step: swe_set_state(pinned host) + swe_step(1) + swe_get_state(pinned host)"}
     zstats = sw.swe_zone_stats(ctx) if args.zones > 0 else None
+    if zstats:
+        zstats["setup_ms"] = sw.swe_zone_setup_ms(ctx)       # row f4: device ghost layers / zone build / whole call
     roofline["fp64_peak_TFLOPs_measured"] = sw.swe_fp64_peak(ctx)      # the other side of the roofline
     sw.swe_mesh_destroy(ctx)
 

@@ -876,25 +876,21 @@ static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, i
     const int nc = (int)c->g.nc;
     const int W = (nz + 63) / 64;
     const size_t words = (size_t)W * nc;
-    int* d_zone = nullptr;
-    unsigned long long *d_reach[2] = {nullptr, nullptr}, *d_fresh[3] = {nullptr, nullptr, nullptr};
-    unsigned long long *d_count = nullptr, *d_keys[2] = {nullptr, nullptr};
-    unsigned int* d_hist = nullptr;
+    // one arena for the masks (two reach buffers, one fresh buffer per layer), the two counters and
+    // the zone ids; a second one, sized once the number of ghosts is known, for the keys
+    unsigned long long *arena = nullptr, *karena = nullptr;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
-    auto cleanup = [&] {
-        cudaFree(d_zone); cudaFree(d_reach[0]); cudaFree(d_reach[1]);
-        for (auto p : d_fresh) cudaFree(p);
-        cudaFree(d_count); cudaFree(d_keys[0]); cudaFree(d_keys[1]); cudaFree(d_hist);
-    };
     keys.clear();
     const int grid = grid_for(nc, c->grid_light);
     unsigned long long total = 0;
-    if (ok(cudaMalloc((void**)&d_zone, (size_t)nc * sizeof(int))) &&
-        ok(cudaMalloc((void**)&d_reach[0], words * 8)) && ok(cudaMalloc((void**)&d_reach[1], words * 8)) &&
-        ok(cudaMalloc((void**)&d_count, 2 * sizeof(unsigned long long)))) {
-        for (int l = 0; l < nlayers; ++l) ok(cudaMalloc((void**)&d_fresh[l], words * 8));
-    }
+    const size_t nmask = (size_t)(2 + nlayers) * words;
+    ok(cudaMalloc((void**)&arena, (nmask + 2) * 8 + (size_t)nc * sizeof(int)));
+    unsigned long long* d_reach[2] = {arena, arena + words};
+    unsigned long long* d_fresh[3] = {nullptr, nullptr, nullptr};
+    for (int l = 0; l < nlayers; ++l) d_fresh[l] = arena + (size_t)(2 + l) * words;
+    unsigned long long* d_count = arena + nmask;             // [0] ghosts found, [1] emit cursor
+    int* d_zone = (int*)(arena + nmask + 2);
     if (e == cudaSuccess) {
         ok(cudaMemcpyAsync(d_zone, zone_of.data(), (size_t)nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         ok(cudaMemsetAsync(d_count, 0, 2 * sizeof(unsigned long long), c->stream));
@@ -906,12 +902,13 @@ static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, i
         ok(cudaMemcpyAsync(&total, d_count, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
         ok(cudaStreamSynchronize(c->stream));
     }
+    if (e == cudaSuccess && total > (unsigned long long)INT32_MAX) { cudaFree(arena); err = "too many ghost cells"; return false; }
     if (e == cudaSuccess && total > 0) {
-        if (total > (unsigned long long)INT32_MAX) { cleanup(); err = "too many ghost cells"; return false; }
         const long long n = (long long)total;
         const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
-        if (ok(cudaMalloc((void**)&d_keys[0], (size_t)n * 8)) && ok(cudaMalloc((void**)&d_keys[1], (size_t)n * 8)) &&
-            ok(cudaMalloc((void**)&d_hist, (size_t)256 * nblk * sizeof(unsigned int)))) {
+        if (ok(cudaMalloc((void**)&karena, (size_t)n * 16 + (size_t)256 * nblk * sizeof(unsigned int)))) {
+            unsigned long long* d_keys[2] = {karena, karena + n};
+            unsigned int* d_hist = (unsigned int*)(karena + 2 * n);
             for (int l = 0; l < nlayers; ++l)
                 k_gl_emit<<<grid, 256, 0, c->stream>>>(d_fresh[l], d_zone, l + 1, nz, nc, W, d_keys[0], d_count + 1);
             // significant key bits: 32 (cell) + those of the largest bucket (nz * nz * 4 - 1)
@@ -932,7 +929,7 @@ static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, i
             ok(cudaStreamSynchronize(c->stream));
         }
     }
-    cleanup();
+    cudaFree(arena); cudaFree(karena);
     if (e != cudaSuccess) { cudaGetLastError(); err = std::string("device ghost-layer generation: ") + cudaGetErrorString(e); return false; }
     return true;
 }
