@@ -101,6 +101,16 @@ int swe_step(swe_ctx* ctx, int nsteps, double cfl, int scheme, double* t_out, do
  * results are identical either way. */
 int swe_set_graphs(swe_ctx* ctx, int on);
 
+/* Cells without water are not worked on (wet/dry treatment of SURVEY.md section 8(c), A.3.5 /
+ * A.6: a cell whose record is (0, 0, 0, z) has zero gradients, and an interior edge between two
+ * such cells a zero flux record).  On the un-zoned mesh swe_step keeps one bit per cell / edge for
+ * "this record holds nothing" (state buffers, gradient buffer, flux buffer; 0.5 bytes per cell in
+ * all) and neither rewrites nor rereads such records from one stage to the next; a cell that is
+ * (0, 0, 0, z) with three zero flux records is left as it is.  The results are bit-identical to the
+ * step that works on every cell (on = 0; default: on).  The bits are rebuilt by the first step
+ * after any other call that may touch the buffers. */
+int swe_set_dry_masks(swe_ctx* ctx, int on);
+
 /* Zone decomposition resident on this GPU.
  *   nzones : number of zones; zone_of_cell (nt, user order, values in [0,nzones)) or NULL =
  *            recursive coordinate bisection (nzones must then be a power of two)

@@ -38,6 +38,7 @@ SIGNATURES = {
     "swe_set_time": (C.c_int, [_vp, C.c_double]),
     "swe_step": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, _dp, _dp]),
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
+    "swe_set_dry_masks": (C.c_int, [_vp, C.c_int]),
     "swe_fp64_peak": (C.c_int, [_vp, _dp]),
     "swe_zones_create": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
@@ -206,6 +207,10 @@ def swe_fp64_peak(ctx):
     v = C.c_double()
     _check(lib().swe_fp64_peak(ctx, C.byref(v)))
     return v.value
+
+
+def swe_set_dry_masks(ctx, on):
+    _check(lib().swe_set_dry_masks(ctx, 1 if on else 0))
 
 
 def swe_set_graphs(ctx, on):

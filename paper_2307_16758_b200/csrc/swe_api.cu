@@ -44,6 +44,8 @@ struct Store {
     std::vector<int32_t> h_btag;
     double4 *A = nullptr, *B = nullptr, *grad = nullptr;
     FluxBuf F{};
+    unsigned *zA = nullptr, *zB = nullptr, *gz = nullptr, *fz = nullptr;   // dry-record bit masks (DryMasks)
+    size_t mask_words = 0;                                               // zA | zB | gz | fz, one allocation
     int64_t nc = 0, ne = 0, nbe = 0;
 
     template <class T> cudaError_t alloc(T** p, size_t n) {
@@ -108,6 +110,13 @@ struct swe_ctx {
     int64_t prof_n[NKIND] = {0};
     // one time step captured as a CUDA graph and replayed (launch-bound on small meshes): valid for
     // one (scheme, cfl, store, parameter set); captured on a side stream, launched on `stream`
+    // dry-record bit masks (swe_kernels.cuh DryMasks): used by swe_step on the un-zoned store only;
+    // `masks_live` = the bits describe the buffers; every other entry point clears it (check_ctx)
+    bool dry_masks = true;
+    mutable bool masks_live = false;
+    int mask_scheme = -1;
+    bool mk_on = false;                // set while swe_step enqueues its stages
+    bool graph_masks = false;
     bool use_graphs = true;
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t step_exec = nullptr;
@@ -219,6 +228,12 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.alloc(&st.F.fyl, (size_t)M.ne));
     CU(st.alloc(&st.F.fxr, (size_t)M.ne));
     CU(st.alloc(&st.F.fyr, (size_t)M.ne));
+    {
+        const size_t wc = ((size_t)M.nc + 31) / 32 + 1, we = ((size_t)M.ne + 31) / 32 + 1;
+        st.mask_words = 3 * wc + we;
+        CU(st.alloc(&st.zA, st.mask_words));
+        st.zB = st.zA + wc; st.gz = st.zB + wc; st.fz = st.gz + wc;
+    }
     CU(cudaMemsetAsync(st.grad, 0, 3 * (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.B, 0, (size_t)M.nc * sizeof(double4), s));
     CU(cudaMemsetAsync(st.d_nman, 0, (size_t)(M.nc ? M.nc : 1) * sizeof(double), s));
@@ -301,6 +316,15 @@ void free_zones(swe_ctx* c) {
 }
 
 // ---- kernel launch helpers (all on c->stream) ----
+// masks of the stage that reads `Uin` and writes `Uout` (either may be nullptr when not needed)
+DryMasks masks_of(const swe_ctx* c, const Store& st, const double4* Uin, const double4* Uout) {
+    DryMasks K{nullptr, nullptr, nullptr, nullptr};
+    if (!c->mk_on) return K;
+    K.zin = (Uin == st.A) ? st.zA : st.zB;
+    K.zout = (Uout == st.A) ? st.zA : st.zB;
+    K.gz = st.gz; K.fz = st.fz;
+    return K;
+}
 void run_dt_reduce(swe_ctx* c, Store& st, const double4* U) {
     launch(c, KIND_DT, [&] {
         k_dt_reduce<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.dm, U, c->P, c->d_S);
@@ -317,16 +341,29 @@ void run_grad(swe_ctx* c, Store& st, const double4* U, int scheme = K_MUSCL) {
     }
     if (scheme != K_MUSCL) return;
     launch(c, KIND_GRAD, [&] {
-        k_grad_limit<<<grid_for(st.nc, c->grid_grad, SWE_GRAD_THREADS), SWE_GRAD_THREADS, 0, c->stream>>>(st.dm, U, st.grad, c->P);
+        const int gr = grid_for(st.nc, c->grid_grad, SWE_GRAD_THREADS);
+        const DryMasks K = masks_of(c, st, U, nullptr);
+        if (c->mk_on) k_grad_limit<true><<<gr, SWE_GRAD_THREADS, 0, c->stream>>>(st.dm, U, st.grad, c->P, K);
+        else k_grad_limit<false><<<gr, SWE_GRAD_THREADS, 0, c->stream>>>(st.dm, U, st.grad, c->P, K);
     });
 }
 void run_flux(swe_ctx* c, Store& st, const double4* U, int scheme) {
     launch(c, KIND_FLUX, [&] {
         const int gr = grid_for(st.ne, c->grid_flux[scheme], SWE_FLUX_THREADS);
-        if (scheme == K_HLLC) k_edge_flux<K_HLLC><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else if (scheme == K_MUSCL) k_edge_flux<K_MUSCL><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else if (scheme == K_WAF) k_edge_flux<K_WAF><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
-        else k_edge_flux<K_MUSCL_MS><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S);
+        const DryMasks K = masks_of(c, st, U, nullptr);
+#define SWE_FLUX_LAUNCH(SC, MK) k_edge_flux<SC, MK><<<gr, SWE_FLUX_THREADS, 0, c->stream>>>(st.dm, U, st.grad, st.F, c->P, c->d_S, K)
+        if (c->mk_on) {
+            if (scheme == K_HLLC) SWE_FLUX_LAUNCH(K_HLLC, true);
+            else if (scheme == K_MUSCL) SWE_FLUX_LAUNCH(K_MUSCL, true);
+            else if (scheme == K_WAF) SWE_FLUX_LAUNCH(K_WAF, true);
+            else SWE_FLUX_LAUNCH(K_MUSCL_MS, true);
+        } else {
+            if (scheme == K_HLLC) SWE_FLUX_LAUNCH(K_HLLC, false);
+            else if (scheme == K_MUSCL) SWE_FLUX_LAUNCH(K_MUSCL, false);
+            else if (scheme == K_WAF) SWE_FLUX_LAUNCH(K_WAF, false);
+            else SWE_FLUX_LAUNCH(K_MUSCL_MS, false);
+        }
+#undef SWE_FLUX_LAUNCH
     });
 }
 // mode 0: Uout = E(Uin); mode 1: Uout = (U0 + E(Uin))/2; fuse: fold the next CFL min in;
@@ -349,10 +386,20 @@ void run_update(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, do
     const int skip = part == 2 ? 1 : 0;
     launch(c, KIND_UPDATE, [&] {
         const int gr = grid_for(st.nc, c->grid_upd);
-        if (mode == 0 && !fuse) k_cell_update<0, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
-        else if (mode == 0) k_cell_update<0, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
-        else if (!fuse) k_cell_update<1, false><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
-        else k_cell_update<1, true><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip);
+        const DryMasks K = masks_of(c, st, Uin, Uout);
+#define SWE_UPD_LAUNCH(MO, FU, MK) k_cell_update<MO, FU, MK><<<gr, 256, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.F, c->P, c->d_S, skip, K)
+        if (c->mk_on) {
+            if (mode == 0 && !fuse) SWE_UPD_LAUNCH(0, false, true);
+            else if (mode == 0) SWE_UPD_LAUNCH(0, true, true);
+            else if (!fuse) SWE_UPD_LAUNCH(1, false, true);
+            else SWE_UPD_LAUNCH(1, true, true);
+        } else {
+            if (mode == 0 && !fuse) SWE_UPD_LAUNCH(0, false, false);
+            else if (mode == 0) SWE_UPD_LAUNCH(0, true, false);
+            else if (!fuse) SWE_UPD_LAUNCH(1, false, false);
+            else SWE_UPD_LAUNCH(1, true, false);
+        }
+#undef SWE_UPD_LAUNCH
     });
 }
 void run_exchange_state(swe_ctx* c, double4* U, int64_t first, int64_t count, bool do_pack, bool do_unpack) {
@@ -399,7 +446,18 @@ int sync_global_from_zoned(swe_ctx* c) {
     return SWE_OK;
 }
 
-int check_ctx(const swe_ctx* c) { return c ? SWE_OK : fail(SWE_ERR_ARG, "null context"); }
+// every entry point comes through here: whatever it does to the buffers, the dry-record masks no
+// longer describe them (swe_step and the read-only getters restore the flag themselves)
+int check_ctx(const swe_ctx* c) {
+    if (!c) return fail(SWE_ERR_ARG, "null context");
+    c->masks_live = false;
+    return SWE_OK;
+}
+struct KeepMasks {                      // read-only entry points
+    const swe_ctx* c; bool live;
+    explicit KeepMasks(const swe_ctx* c_) : c(c_), live(c_ && c_->masks_live) {}
+    ~KeepMasks() { if (c) c->masks_live = live; }
+};
 
 }  // namespace
 
@@ -450,12 +508,12 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
         return nbk * c->num_sm;
     };
     c->grid_light = 8 * c->num_sm;
-    c->grid_grad = occ((const void*)k_grad_limit, 4, SWE_GRAD_THREADS);
-    c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC>, 4, SWE_FLUX_THREADS);
-    c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL>, 2, SWE_FLUX_THREADS);
-    c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF>, 2, SWE_FLUX_THREADS);
-    c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS>, 2, SWE_FLUX_THREADS);
-    c->grid_upd = occ((const void*)k_cell_update<1, true>, 4);
+    c->grid_grad = occ((const void*)k_grad_limit<false>, 4, SWE_GRAD_THREADS);
+    c->grid_flux[K_HLLC] = occ((const void*)k_edge_flux<K_HLLC, false>, 4, SWE_FLUX_THREADS);
+    c->grid_flux[K_MUSCL] = occ((const void*)k_edge_flux<K_MUSCL, false>, 2, SWE_FLUX_THREADS);
+    c->grid_flux[K_WAF] = occ((const void*)k_edge_flux<K_WAF, false>, 2, SWE_FLUX_THREADS);
+    c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS, false>, 2, SWE_FLUX_THREADS);
+    c->grid_upd = occ((const void*)k_cell_update<1, true, false>, 4);
     c->grid_ms = occ((const void*)k_ms_slopes, 5, 128);
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
@@ -499,6 +557,7 @@ int swe_mesh_destroy(swe_ctx* c) {
 }
 
 int swe_mesh_info(const swe_ctx* c, int64_t* ncell, int64_t* nedge, int64_t* nbedge, double* min_inradius) {
+    KeepMasks keep_masks(c);   // read-only
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (ncell) *ncell = c->H.nt;
     if (nedge) *nedge = c->H.m.ne;
@@ -585,6 +644,7 @@ int swe_set_state(swe_ctx* c, const double* h, const double* hu, const double* h
 }
 
 int swe_get_state(const swe_ctx* cc, double* h, double* hu, double* hv) {
+    KeepMasks keep_masks(cc);   // read-only
     swe_ctx* c = const_cast<swe_ctx*>(cc);
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!h || !hu || !hv) return fail(SWE_ERR_ARG, "NULL state array");
@@ -621,6 +681,7 @@ int swe_set_time(swe_ctx* c, double t) {
 }
 
 int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, double* last_dt_out) {
+    const bool masks_were_live = c && c->masks_live;
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (nsteps < 0 || !(cfl > 0.0) || scheme < 0 || scheme > 3) return fail(SWE_ERR_ARG, "bad step arguments");
     if (c->has_zones && c->Z.nranks > 1)
@@ -628,6 +689,15 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
     if (c->has_zones && (scheme == K_WAF || scheme == K_MUSCL_MS) && c->Z.nlayers < 2)
         return fail(SWE_ERR_STATE, "WAF and the multislope MUSCL need zones with at least 2 ghost layers");
     Store& st = c->active();
+    // dry-record masks: un-zoned store only; cleared unless the previous call on this context was a
+    // swe_step with the same scheme (the gradient buffer holds other records for the multislope pass)
+    struct MaskScope { swe_ctx* c; ~MaskScope() { c->mk_on = false; } } mask_scope{c};
+    c->mk_on = c->dry_masks && !c->has_zones && nsteps > 0;
+    if (c->mk_on) {
+        if (!masks_were_live || c->mask_scheme != scheme)
+            CU(cudaMemsetAsync(st.zA, 0, st.mask_words * sizeof(unsigned), c->stream));
+        c->mask_scheme = scheme;
+    }
     auto enqueue_step = [&] {
         launch(c, KIND_MISC, [&] { k_dt_finalize<<<1, 1, 0, c->stream>>>(c->d_S, cfl, 1); });
         if (scheme == K_MUSCL || scheme == K_MUSCL_MS) {                    // Heun RK2 (A.11)
@@ -644,7 +714,8 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
     }
     if (c->use_graphs && !c->profile && nsteps >= 2) {
         // capture one step (same kernels, same order, same arguments) and replay it
-        if (!c->step_exec || c->graph_scheme != scheme || c->graph_cfl != cfl || c->graph_zoned != c->has_zones) {
+        if (!c->step_exec || c->graph_scheme != scheme || c->graph_cfl != cfl || c->graph_zoned != c->has_zones ||
+            c->graph_masks != c->mk_on) {
             drop_graph(c);
             if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
             const int64_t l0 = c->launches, h0 = c->halo_bytes;
@@ -662,7 +733,7 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
             if (e == cudaSuccess) e = cudaGraphInstantiate(&c->step_exec, graph, 0);
             if (graph) cudaGraphDestroy(graph);
             if (e != cudaSuccess) { c->step_exec = nullptr; return fail(SWE_ERR_CUDA, std::string("step graph: ") + cudaGetErrorString(e)); }
-            c->graph_scheme = scheme; c->graph_cfl = cfl; c->graph_zoned = c->has_zones;
+            c->graph_scheme = scheme; c->graph_cfl = cfl; c->graph_zoned = c->has_zones; c->graph_masks = c->mk_on;
         }
         for (; s0 < nsteps; ++s0) {
             CU(cudaGraphLaunch(c->step_exec, c->stream));
@@ -675,6 +746,7 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
         c->steps++;
     }
     CU(cudaGetLastError());
+    c->masks_live = c->mk_on;
     if (c->profile) profile_collect(c);
     if (t_out || last_dt_out) {
         StepScalars hs;
@@ -711,6 +783,12 @@ int swe_fp64_peak(swe_ctx* c, double* tflops_out) {
     return SWE_OK;
 }
 
+int swe_set_dry_masks(swe_ctx* c, int on) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    c->dry_masks = on != 0;
+    return SWE_OK;
+}
+
 int swe_set_graphs(swe_ctx* c, int on) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     c->use_graphs = on != 0;
@@ -719,7 +797,9 @@ int swe_set_graphs(swe_ctx* c, int on) {
 }
 
 int swe_step_timed(swe_ctx* c, int nsteps, double cfl, int scheme, float* ms_out) {
+    const bool live = c && c->masks_live;
     if (check_ctx(c)) return SWE_ERR_ARG;
+    c->masks_live = live;               // swe_step with two events around it: nothing else touches the buffers
     cudaEvent_t a, b;
     CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
     CU(cudaEventRecord(a, c->stream));
@@ -861,6 +941,7 @@ int swe_euler_stage(swe_ctx* c, double dt, int scheme, double* h1, double* hu1, 
 }
 
 int swe_get_stats(const swe_ctx* c, int64_t* steps, int64_t* kernel_launches, int64_t* halo_bytes) {
+    KeepMasks keep_masks(c);   // read-only
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (steps) *steps = c->steps;
     if (kernel_launches) *kernel_launches = c->launches;
@@ -1211,6 +1292,7 @@ int swe_dist_stage(swe_ctx* c, int scheme, int stage) {
 }
 
 int swe_get_time(swe_ctx* c, double* t_out, double* last_dt_out) {
+    KeepMasks keep_masks(c);   // read-only
     if (check_ctx(c)) return SWE_ERR_ARG;
     StepScalars hs;
     CU(cudaMemcpyAsync(&hs, c->d_S, sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
