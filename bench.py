@@ -339,8 +339,8 @@ def main():
                     help="run the distributed arm (DistSolver, zones over ranks) even with a single rank")
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-dry-masks", action="store_true",
-                    help="work on every cell every stage (swe_set_dry_masks off): the A/B for the dry-record bit masks")
+    ap.add_argument("--dry-masks", action="store_true",
+                    help="swe_set_dry_masks on: leave the records of cells / edges without water alone (un-zoned mesh only)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -374,8 +374,8 @@ def main():
     nt = info["ncell"]
     if args.zones > 0:
         sw.swe_zones_create(ctx, args.zones, args.layers)
-    if args.no_dry_masks:
-        sw.swe_set_dry_masks(ctx, False)
+    if args.dry_masks:
+        sw.swe_set_dry_masks(ctx, True)
 
     # ---- device-resident throughput: warm-up, then exactly K timed steps ----
     sw.swe_step(ctx, args.warmup, cfl, args.scheme)
@@ -399,7 +399,8 @@ def main():
     sw.swe_set_profile(ctx, False)
     clocks = clk.stop()
     peak, peak_src = hbm_peak()
-    roofline = kernel_roofline(prof, args.steps, args.scheme, nt, ms / args.steps, peak, peak_src, args.workload)
+    roofline = kernel_roofline(prof, args.steps, args.scheme, nt, ms / args.steps, peak, peak_src,
+                               args.workload + ("+masks" if args.dry_masks and args.zones == 0 else ""))
 
     # ---- end to end through the C ABI with HOST buffers: every step copies the state host->device
     # (pinned memory), advances one step and reads the state back ----
@@ -448,7 +449,7 @@ def main():
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
                        "zones": args.zones, "ghost_layers": args.layers if args.zones else 0,
                        "renumber": args.renumber,
-                       "dry_masks": (not args.no_dry_masks) and args.zones == 0, "paper_context": PAPER_CONTEXT[args.scheme]},
+                       "dry_masks": args.dry_masks and args.zones == 0, "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
             "gpu_launches": l1["kernel_launches"] - l0["kernel_launches"], "clocks": clocks,
         }

@@ -107,8 +107,10 @@ int swe_set_graphs(swe_ctx* ctx, int on);
  * "this record holds nothing" (state buffers, gradient buffer, flux buffer; 0.5 bytes per cell in
  * all) and neither rewrites nor rereads such records from one stage to the next; a cell that is
  * (0, 0, 0, z) with three zero flux records is left as it is.  The results are bit-identical to the
- * step that works on every cell (on = 0; default: on).  The bits are rebuilt by the first step
- * after any other call that may touch the buffers. */
+ * step that works on every cell (on = 0, the default).  The bits are rebuilt by the first step
+ * after any other call that may touch the buffers.  Opt-in because it pays only on meshes with
+ * large dry areas, and less than the bytes it saves: on configs[3] the step
+ * moves 22 % fewer bytes and takes 5 % less time; with every cell wet it costs 4-5 %. */
 int swe_set_dry_masks(swe_ctx* ctx, int on);
 
 /* Zone decomposition resident on this GPU.

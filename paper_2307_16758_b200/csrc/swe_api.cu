@@ -112,7 +112,7 @@ struct swe_ctx {
     // one (scheme, cfl, store, parameter set); captured on a side stream, launched on `stream`
     // dry-record bit masks (swe_kernels.cuh DryMasks): used by swe_step on the un-zoned store only;
     // `masks_live` = the bits describe the buffers; every other entry point clears it (check_ctx)
-    bool dry_masks = true;
+    bool dry_masks = false;            // opt-in (swe_set_dry_masks): see DESIGN.md section 6
     mutable bool masks_live = false;
     int mask_scheme = -1;
     bool mk_on = false;                // set while swe_step enqueues its stages
