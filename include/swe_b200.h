@@ -238,6 +238,13 @@ int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_o
  * thread, 8 blocks of 256 threads per SM, best of 3 timed launches): the ALU-side roofline the
  * bandwidth-bound claim is checked against.  Synchronises. */
 int swe_fp64_peak(swe_ctx* ctx, double* tflops_out);
+
+/* Test interface: the kernels' own division and square-root sequences (MUFU seed + one Newton step +
+ * residual correction, swe_kernels.cuh) against the IEEE-rounded a[i] / x[i] and sqrt(x[i]) on n
+ * caller-supplied samples (host or device pointers; x > 0, everything in the normal range).
+ * ndiff[0], ndiff[1]: how many quotients / roots differ from the IEEE result; maxrel[0], maxrel[1]:
+ * the largest relative difference of each.  Errors: SWE_ERR_ARG, SWE_ERR_CUDA. */
+int swe_fastmath_check(swe_ctx* ctx, int64_t n, const double* a, const double* x, int64_t* ndiff, double* maxrel);
 /* per-kernel timing: runs `reps` launches of one kernel of the hot path on the current state
  * between two events; which: 0 dt_reduce, 1 grad_limit (scheme SWE_MUSCL_MS: the multislope side
  * records, k_ms_slopes), 2 edge_flux(scheme), 3 cell_update (Euler

@@ -40,6 +40,7 @@ SIGNATURES = {
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
     "swe_set_dry_masks": (C.c_int, [_vp, C.c_int]),
     "swe_fp64_peak": (C.c_int, [_vp, _dp]),
+    "swe_fastmath_check": (C.c_int, [_vp, C.c_int64, _vp, _vp, _i64p, _dp]),
     "swe_zones_create": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_unpack_ghosts": (C.c_int, [_vp, C.c_int]),
@@ -201,6 +202,14 @@ def swe_step(ctx, nsteps, cfl, scheme, sync=True):
     t, dt = C.c_double(), C.c_double()
     _check(lib().swe_step(ctx, int(nsteps), float(cfl), _scheme(scheme), C.byref(t), C.byref(dt)))
     return t.value, dt.value
+
+
+def swe_fastmath_check(ctx, a, x):
+    a, x = _f64(a), _f64(x)
+    nd = (C.c_int64 * 2)()
+    mr = (C.c_double * 2)()
+    _check(lib().swe_fastmath_check(ctx, a.size, _ptr(a), _ptr(x), nd, mr))
+    return {"div_differs": nd[0], "sqrt_differs": nd[1], "div_maxrel": mr[0], "sqrt_maxrel": mr[1]}
 
 
 def swe_fp64_peak(ctx):

@@ -783,6 +783,35 @@ int swe_fp64_peak(swe_ctx* c, double* tflops_out) {
     return SWE_OK;
 }
 
+int swe_fastmath_check(swe_ctx* c, int64_t n, const double* a, const double* x, int64_t* ndiff /*2*/, double* maxrel /*2*/) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (n <= 0 || !a || !x || !ndiff || !maxrel) return fail(SWE_ERR_ARG, "bad fastmath_check arguments");
+    double *da = nullptr, *dx = nullptr;
+    unsigned long long* dout = nullptr;
+    const bool dev = is_device_ptr(a) && is_device_ptr(x);
+    if (!dev) {
+        CU(cudaMalloc((void**)&da, (size_t)n * sizeof(double)));
+        cudaError_t e = cudaMalloc((void**)&dx, (size_t)n * sizeof(double));
+        if (e != cudaSuccess) { cudaFree(da); return fail(SWE_ERR_CUDA, cudaGetErrorString(e)); }
+        cudaMemcpyAsync(da, a, (size_t)n * sizeof(double), cudaMemcpyDefault, c->stream);
+        cudaMemcpyAsync(dx, x, (size_t)n * sizeof(double), cudaMemcpyDefault, c->stream);
+    }
+    cudaError_t e = cudaMalloc((void**)&dout, 4 * sizeof(unsigned long long));
+    unsigned long long h[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess) {
+        cudaMemsetAsync(dout, 0, sizeof(h), c->stream);
+        k_fastmath_check<<<grid_for(n, c->grid_light), 256, 0, c->stream>>>(dev ? a : da, dev ? x : dx, (long long)n, dout);
+        c->launches++;
+        cudaMemcpyAsync(h, dout, sizeof(h), cudaMemcpyDeviceToHost, c->stream);
+        e = cudaStreamSynchronize(c->stream);
+    }
+    cudaFree(da); cudaFree(dx); cudaFree(dout);
+    if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    ndiff[0] = (int64_t)h[0]; ndiff[1] = (int64_t)h[1];
+    memcpy(&maxrel[0], &h[2], sizeof(double)); memcpy(&maxrel[1], &h[3], sizeof(double));
+    return SWE_OK;
+}
+
 int swe_set_dry_masks(swe_ctx* c, int on) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     c->dry_masks = on != 0;
