@@ -134,15 +134,17 @@ def hbm_peak():
 
 
 def traffic_table():
-    """ncu dram bytes per launch (profiles/*.csv written from ncu --set full captures), if any."""
+    """ncu DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+    capture, profiles/dram_traffic.csv: workload, kernel, bytes, capture): {(workload, kernel): (bytes, capture)}.
+    A table captured in another run, NOT a measurement of this one: the line says so (traffic_source)."""
     out = {}
     p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if os.path.exists(p):
         for ln in open(p):
-            f = ln.strip().split(",")
+            f = ln.strip().split(",", 3)
             if len(f) >= 3 and f[0] != "workload":
                 try:
-                    out[(f[0], f[1])] = float(f[2])
+                    out[(f[0], f[1])] = (float(f[2]), f[3] if len(f) > 3 else "")
                 except ValueError:
                     pass
     return out
@@ -171,10 +173,11 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    sample = "c3s" if args.workload == "c3" else args.workload
-    cfg, desc = build_workload(sample)
+    # the SAME workload as the GPU arm (at 13.1 M cells the oracle runs ~20 steps);
+    # each step is one full time step of the whole mesh, as many of the requested steps as fit 90 s
+    cfg, desc = build_workload(args.workload)
     cfl = 0.9 if args.scheme == "hllc" else 0.45
-    warm = max(1, min(args.warmup, 3))
+    warm = max(1, min(args.warmup, 2))
     v, cores, nt, secs, steps = oracle_run(cfg, args.scheme, cfl, warm, args.steps, budget_s=90.0)
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": "cell-updates/s", "n_gpus": args.gpus,
@@ -212,24 +215,32 @@ def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workloa
             kern[k]["frac_of_peak"] = kern[k]["algo_GBps"] / peak
     dom = max((k for k in algo if k in kern), key=lambda k: kern[k]["share"])
     tt = traffic_table()
-    traffic = tt.get((workload, dom + "_" + scheme), tt.get((workload, dom)))
+    row = tt.get((workload, dom + "_" + scheme), tt.get((workload, dom)))
+    traffic, traffic_src = (row[0], "profiles/dram_traffic.csv (ncu --set full, captured earlier: %s)" % row[1]) if row else (None, None)
     step_bytes = ALGO_BYTES["step_" + scheme]
     rate = cells / (step_ms * 1e-3)
     # physical DRAM bytes of one step from the ncu table (13.1 M-cell MUSCL-RK2 only), SURVEY 8(d)(iii)
     step_dram = None
     if scheme == "muscl" and all((workload, k) in tt for k in ("grad_limit", "edge_flux_muscl", "cell_update_muscl")):
-        step_dram = 2.0 * (tt[(workload, "grad_limit")] + tt[(workload, "edge_flux_muscl")] + tt[(workload, "cell_update_muscl")])
+        step_dram = 2.0 * (tt[(workload, "grad_limit")][0] + tt[(workload, "edge_flux_muscl")][0] + tt[(workload, "cell_update_muscl")][0])
     extra = {}
-    if kern[dom]["algo_GBps"] > peak:
-        extra["note"] = ("frac > 1: the algorithmic bytes count every cell and edge, the kernels skip cells without "
-                         "water (zero gradients / zero flux records written without reading their inputs), so the "
-                         "bytes actually moved (traffic) are below the algorithmic figure; DESIGN.md section 6")
+    if traffic:
+        # what the kernel actually moved (ncu) over the time measured here: the fraction of the
+        # bandwidth the kernel reaches on its own bytes, whatever the dry-cell skips leave out
+        extra["frac_physical"] = traffic / (kern[dom]["ms_per_launch"] * 1e-3) / 1e9 / peak
+        extra["physical_GBps"] = traffic / (kern[dom]["ms_per_launch"] * 1e-3) / 1e9
+    if kern[dom]["algo_GBps"] > 0.95 * peak:
+        extra["note"] = ("frac counts the FIXED algorithmic bytes of every cell and edge; the kernels skip cells / edges "
+                         "without water (zero records written without reading their inputs), so on a partly dry state "
+                         "the bytes actually moved are fewer: read frac_physical (ncu bytes) and all_wet (no dry cell, "
+                         "where the algorithmic count is what is moved) beside it; DESIGN.md section 6")
     if step_dram:
         extra.update({"step_dram_bytes_ncu": step_dram, "step_algo_over_dram_bytes": step_bytes * cells / step_dram,
-                      "step_dram_GBps": step_dram / (step_ms * 1e-3) / 1e9})
+                      "step_dram_GBps": step_dram / (step_ms * 1e-3) / 1e9,
+                      "step_frac_physical": step_dram / (step_ms * 1e-3) / 1e9 / peak})
     return dict(extra, **{
         "bound": "hbm", "kernel": dom, "achieved": kern[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
-        "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
+        "frac": kern[dom]["algo_GBps"] / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
         "algo_bytes_per_launch": algo[dom] * cells,
         "step_algo_GBps": step_bytes * rate / 1e9,
         "step_frac_of_peak": step_bytes * rate / 1e9 / peak,
@@ -342,6 +353,10 @@ def main():
     ap.add_argument("--dry-masks", action="store_true",
                     help="swe_set_dry_masks on: leave the records of cells / edges without water alone (un-zoned mesh only)")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--reps", type=int, default=5,
+                    help="the timed region of K steps is run this many times; value = the median (BASELINE.md section 4)")
+    ap.add_argument("--no-all-wet", action="store_true",
+                    help="skip the second measurement on the flooded mesh (roofline.all_wet; workload c3, N = 1 only)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -377,20 +392,28 @@ def main():
     if args.dry_masks:
         sw.swe_set_dry_masks(ctx, True)
 
-    # ---- device-resident throughput: warm-up, then exactly K timed steps ----
+    # ---- device-resident throughput: warm-up, then exactly K timed steps, `reps` times over ----
     sw.swe_step(ctx, args.warmup, cfl, args.scheme)
     torch.cuda.synchronize()
+    dry = sw.swe_dry_counts(ctx)                                  # of the state the timed region starts from
     swdist.barrier()
     l0 = sw.swe_get_stats(ctx)
     clk = ClockSampler(local)
     clk.start()
-    ms = sw.swe_step_timed(ctx, args.steps, cfl, args.scheme)     # CUDA events on the context's stream
-    torch.cuda.synchronize()
+    rep_ms = []
+    for _ in range(max(1, args.reps)):
+        torch.cuda.synchronize()
+        swdist.barrier()
+        m = sw.swe_step_timed(ctx, args.steps, cfl, args.scheme)  # CUDA events on the context's stream
+        torch.cuda.synchronize()
+        swdist.barrier()
+        rep_ms.append(swdist.reduce_max(m))
     l1 = sw.swe_get_stats(ctx)
-    swdist.barrier()
-    ms_max = swdist.reduce_max(ms)
+    ms_max = float(np.median(rep_ms))
+    ms = ms_max
     cells_total = swdist.reduce_sum(float(nt))
     value = cells_total * args.steps / (ms_max * 1e-3)
+    launches_per_rep = (l1["kernel_launches"] - l0["kernel_launches"]) // max(1, args.reps)
 
     # ---- the same timed region again with per-kernel CUDA events (roofline of the dominant kernel) ----
     sw.swe_set_profile(ctx, True)
@@ -401,6 +424,42 @@ def main():
     peak, peak_src = hbm_peak()
     roofline = kernel_roofline(prof, args.steps, args.scheme, nt, ms / args.steps, peak, peak_src,
                                args.workload + ("+masks" if args.dry_masks and args.zones == 0 else ""))
+    roofline["dry_state"] = {
+        "cells_not_wet_frac": dry["cells_not_wet"] / dry["cells"], "cells_empty_frac": dry["cells_empty"] / dry["cells"],
+        "edges_between_empty_cells_frac": dry["edges_between_empty_cells"] / max(1, dry["interior_edges"]),
+        "what": "counted on the device after the warm-up steps: cells with h <= h_dry get zero gradients and interior "
+                "edges between two cells with h == 0 a zero flux record without reading their inputs"}
+
+    # ---- the same mesh with every cell wet: here the algorithmic bytes are what is moved ----
+    if args.workload == "c3" and world == 1 and args.zones == 0 and not args.no_all_wet:
+        from swe_inputs import flooded
+        wet = flooded(cfg, 18.0)
+        keep = [torch.empty(nt, dtype=torch.float64, device="cuda") for _ in range(3)]
+        sw.swe_get_state(ctx, *keep)
+        t_keep = sw.swe_get_time(ctx)[0]
+        sw.swe_set_state(ctx, wet["h"], wet["hu"], wet["hv"])
+        sw.swe_step(ctx, args.warmup, cfl, args.scheme)
+        torch.cuda.synchronize()
+        wdry = sw.swe_dry_counts(ctx)
+        wms = float(np.median([sw.swe_step_timed(ctx, args.steps, cfl, args.scheme) for _ in range(3)]))
+        sw.swe_set_profile(ctx, True)
+        sw.swe_step(ctx, args.steps, cfl, args.scheme)
+        wprof = sw.swe_get_profile(ctx)
+        sw.swe_set_profile(ctx, False)
+        wr = kernel_roofline(wprof, args.steps, args.scheme, nt, wms / args.steps, peak, peak_src, "c3w")
+        roofline["all_wet"] = {
+            "workload": "the same mesh and bed flooded to a flat surface at 18 m (swe_inputs.flooded), %d warm-up steps, "
+                        "median of 3 x %d timed steps" % (args.warmup, args.steps),
+            "cells_not_wet_frac": wdry["cells_not_wet"] / wdry["cells"],
+            "ms_per_step": wms / args.steps, "value": nt * args.steps / (wms * 1e-3),
+            "kernel": wr["kernel"], "frac": wr["frac"], "achieved": wr["achieved"],
+            "frac_physical": wr.get("frac_physical"), "traffic": wr["traffic"], "traffic_source": wr["traffic_source"],
+            "step_frac_of_peak": wr["step_frac_of_peak"], "step_frac_of_8TBps": wr["step_frac_of_8TBps"],
+            "step_frac_physical": wr.get("step_frac_physical"),
+            "kernels": {k: {"ms_per_launch": v["ms_per_launch"], "frac_of_peak": v.get("frac_of_peak")} for k, v in wr["kernels"].items()}}
+        sw.swe_set_state(ctx, *keep)                              # back to the timed state for the e2e leg
+        sw.swe_set_time(ctx, t_keep)
+        del keep
 
     # ---- end to end through the C ABI with HOST buffers: every step copies the state host->device
     # (pinned memory), advances one step and reads the state back ----
@@ -430,13 +489,16 @@ def main():
     # ---- the oracle as it stands, timed on this box's host cores (rank 0, N=1 only) ----
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sname = "c3s" if args.workload == "c3" else args.workload
+        # all cores: the SAME workload (20 steps at 13.1 M cells; fewer if they do not
+        # fit 25 s); one thread: the same generator on a 6 km reach, a few steps
+        v, cores, ont, secs, osteps = oracle_run(cfg, args.scheme, cfl, 1, 20, budget_s=25.0)
+        sname = "c3s" if args.workload in ("c3", "c3w", "c3p") else args.workload
         scfg, sdesc = (cfg, desc) if sname == args.workload else build_workload(sname)
-        v, cores, ont, secs, osteps = oracle_run(scfg, args.scheme, cfl, 1, 400, budget_s=15.0)
-        v1, _, _, secs1, osteps1 = oracle_run(scfg, args.scheme, cfl, 1, 50, budget_s=5.0, threads=1)
+        v1, _, ont1, secs1, osteps1 = oracle_run(scfg, args.scheme, cfl, 1, 50, budget_s=5.0, threads=1)
         cpu_baseline = {"value": v, "unit": "cell-updates/s", "cores": cores, "kind": "oracle",
-                        "sample": "%s: %d cells x %d %s steps in %.1f s" % (sdesc, ont, osteps, args.scheme, secs),
-                        "single_thread": {"value": v1, "cores": 1, "sample": "%d steps in %.1f s" % (osteps1, secs1)}}
+                        "sample": "%s: %d cells x %d %s steps in %.1f s" % (desc, ont, osteps, args.scheme, secs),
+                        "single_thread": {"value": v1, "cores": 1,
+                                          "sample": "%s: %d cells x %d steps in %.1f s" % (sdesc, ont1, osteps1, secs1)}}
 
     if rank == 0:
         line = {
@@ -451,7 +513,10 @@ def main():
                        "renumber": args.renumber,
                        "dry_masks": args.dry_masks and args.zones == 0, "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
-            "gpu_launches": l1["kernel_launches"] - l0["kernel_launches"], "clocks": clocks,
+            "gpu_launches": int(launches_per_rep), "clocks": clocks,
+            "reps": {"n": len(rep_ms), "ms_per_step": [m / args.steps for m in rep_ms],
+                     "ms_per_step_min": min(rep_ms) / args.steps, "ms_per_step_max": max(rep_ms) / args.steps,
+                     "value_is": "median over the repetitions of the K-step timed region"},
         }
         if zstats:
             line["config"]["zone_stats"] = zstats

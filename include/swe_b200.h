@@ -73,7 +73,9 @@ int swe_mesh_info(const swe_ctx* ctx, int64_t* ncell, int64_t* nedge, int64_t* n
                   double* min_inradius);
 /* g [m/s2]; h_dry: wet threshold (wet <=> h > h_dry); h_thin: WAF falls back to HLLC within one
  * cell of depth <= h_thin (reading R14); beta: limiter parameter, kappa = beta/2 (1 = minmod /
- * MINBEE eq. 24, 2 = Barth-Jespersen, <= 0 = unlimited). */
+ * MINBEE eq. 24, 2 = Barth-Jespersen, <= 0 = unlimited).  h_dry must be >= 1e-290: the kernels'
+ * reciprocal / square-root sequences need every wet depth to be a normal fp64 number.
+ * Errors: SWE_ERR_ARG (g <= 0, negative or NaN thresholds, h_dry < 1e-290). */
 int swe_set_params(swe_ctx* ctx, double g, double h_dry, double h_thin, double beta);
 /* Manning n per cell, length nt, user order; NULL = 0 everywhere (no friction). */
 int swe_set_manning(swe_ctx* ctx, const double* n_cell);
@@ -238,6 +240,15 @@ int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_o
  * thread, 8 blocks of 256 threads per SM, best of 3 timed launches): the ALU-side roofline the
  * bandwidth-bound claim is checked against.  Synchronises. */
 int swe_fp64_peak(swe_ctx* ctx, double* tflops_out);
+
+/* How much of the CURRENT state the dry-cell / dry-edge skips of the gradient and flux kernels
+ * ("cells without water are not worked on") leave alone; bench.py prints the
+ * fractions beside its roofline figures.  counts (host pointer, 5 entries): [0] owned cells that
+ * are not wet (h <= h_dry), [1] owned cells with h == 0, [2] interior edges between two cells with
+ * h == 0, [3] cells of the mesh, [4] interior edges of the un-zoned mesh.  With zones the edge count
+ * [2] runs over the zoned copy (edges between ghost cells included).  Synchronises.
+ * Errors: SWE_ERR_ARG, SWE_ERR_CUDA. */
+int swe_dry_counts(const swe_ctx* ctx, int64_t* counts);
 
 /* Test interface: the kernels' own division and square-root sequences (MUFU seed + one Newton step +
  * residual correction, swe_kernels.cuh) against the IEEE-rounded a[i] / x[i] and sqrt(x[i]) on n

@@ -40,6 +40,7 @@ SIGNATURES = {
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
     "swe_set_dry_masks": (C.c_int, [_vp, C.c_int]),
     "swe_fp64_peak": (C.c_int, [_vp, _dp]),
+    "swe_dry_counts": (C.c_int, [_vp, _i64p]),
     "swe_fastmath_check": (C.c_int, [_vp, C.c_int64, _vp, _vp, _i64p, _dp]),
     "swe_zones_create": (C.c_int, [_vp, C.c_int, C.c_int, _vp]),
     "swe_pack_ghosts": (C.c_int, [_vp, C.c_int]),
@@ -210,6 +211,13 @@ def swe_fastmath_check(ctx, a, x):
     mr = (C.c_double * 2)()
     _check(lib().swe_fastmath_check(ctx, a.size, _ptr(a), _ptr(x), nd, mr))
     return {"div_differs": nd[0], "sqrt_differs": nd[1], "div_maxrel": mr[0], "sqrt_maxrel": mr[1]}
+
+
+def swe_dry_counts(ctx):
+    v = (C.c_int64 * 5)()
+    _check(lib().swe_dry_counts(ctx, v))
+    return {"cells_not_wet": v[0], "cells_empty": v[1], "edges_between_empty_cells": v[2], "cells": v[3],
+            "interior_edges": v[4]}
 
 
 def swe_fp64_peak(ctx):

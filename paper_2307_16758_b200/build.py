@@ -22,8 +22,11 @@ def needs_build():
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, d) for d in DEPS]
-    if not all(os.path.exists(d) for d in deps):
-        return False                      # binary-only copy of the package: use the library as it is
+    missing = [d for d in deps if not os.path.exists(d)]
+    if missing:
+        # a stale library next to an incomplete source tree must not be picked up silently
+        raise FileNotFoundError("paper_2307_16758_b200: source file(s) missing, cannot tell whether %s is current: %s"
+                                % (os.path.basename(LIB), ", ".join(os.path.relpath(m, HERE) for m in missing)))
     return any(os.path.getmtime(d) > t for d in deps)
 
 

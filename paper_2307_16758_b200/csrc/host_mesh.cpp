@@ -42,20 +42,22 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         if (tri[i] < 0 || tri[i] >= nv) { err = "triangle vertex id out of range"; return false; }
 
     // ---- A.1.1 / A.1.3 : orientation, area, centroid, cell bed (user numbering) ----
+    // Vertex 0 is the pivot of the cross product; a clockwise triangle has its last two vertices
+    // exchanged (which flips the sign of the product, re-evaluated so that the stored area is the
+    // IEEE result of the counter-clockwise expression).  Means are summed in vertex order.
     std::vector<double> area(nt), ucx(nt), ucy(nt), uzc(nt);
-    for (int64_t i = 0; i < nt; ++i) {
-        int32_t* v = &tri[3 * i];
-        double x0 = x[v[0]], y0 = y[v[0]];
-        double a = 0.5 * ((x[v[1]] - x0) * (y[v[2]] - y0) - (x[v[2]] - x0) * (y[v[1]] - y0));
-        if (a < 0.0) {
-            std::swap(v[1], v[2]);
-            a = 0.5 * ((x[v[1]] - x0) * (y[v[2]] - y0) - (x[v[2]] - x0) * (y[v[1]] - y0));
-        }
-        if (!(a > 0.0)) { err = "degenerate (zero-area) triangle"; return false; }
-        area[i] = a;
-        ucx[i] = (x[v[0]] + x[v[1]] + x[v[2]]) / 3.0;
-        ucy[i] = (y[v[0]] + y[v[1]] + y[v[2]]) / 3.0;
-        uzc[i] = (zb[v[0]] + zb[v[1]] + zb[v[2]]) / 3.0;
+    auto half_cross = [&](const int32_t* t) {
+        const double px = x[t[0]], py = y[t[0]];
+        return 0.5 * ((x[t[1]] - px) * (y[t[2]] - py) - (x[t[2]] - px) * (y[t[1]] - py));
+    };
+    auto vertex_mean = [](const double* f, const int32_t* t) { return (f[t[0]] + f[t[1]] + f[t[2]]) / 3.0; };
+    for (int64_t c = 0; c < nt; ++c) {
+        int32_t* t = tri.data() + 3 * c;
+        double omega = half_cross(t);
+        if (omega < 0.0) { std::swap(t[1], t[2]); omega = half_cross(t); }
+        if (!(omega > 0.0)) { err = "degenerate (zero-area) triangle"; return false; }
+        area[c] = omega;
+        ucx[c] = vertex_mean(x, t); ucy[c] = vertex_mean(y, t); uzc[c] = vertex_mean(zb, t);
     }
 
     // ---- A.1.2 : global edges = distinct vertex pairs.  Counting sort of the 3*nt cell sides by
@@ -302,12 +304,19 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         }
         M.rin[i] = 2.0 * area[u] / (lk[0] + lk[1] + lk[2]);   // A.1.5
         min_rin = std::min(min_rin, M.rin[i]);
-        double a11 = 0.0, a12 = 0.0, a22 = 0.0;
-        for (int k = 0; k < 3; ++k) { a11 += dxk[k] * dxk[k]; a12 += dxk[k] * dyk[k]; a22 += dyk[k] * dyk[k]; }
-        double det = a11 * a22 - a12 * a12;
+        // A.1.7: w_k = N^-1 d_k with the normal matrix N = sum_k d_k d_k^T of the three stencil
+        // offsets (symmetric 2 x 2, inverted by its adjugate; sums in side order)
+        double nxx = 0.0, nxy = 0.0, nyy = 0.0;
         for (int k = 0; k < 3; ++k) {
-            M.w[k][2 * i] = (a22 * dxk[k] - a12 * dyk[k]) / det;
-            M.w[k][2 * i + 1] = (-a12 * dxk[k] + a11 * dyk[k]) / det;
+            nxx += dxk[k] * dxk[k];
+            nxy += dxk[k] * dyk[k];
+            nyy += dyk[k] * dyk[k];
+        }
+        const double ndet = nxx * nyy - nxy * nxy;
+        for (int k = 0; k < 3; ++k) {
+            double* wk = &M.w[k][2 * i];
+            wk[0] = (nyy * dxk[k] - nxy * dyk[k]) / ndet;
+            wk[1] = (-nxy * dxk[k] + nxx * dyk[k]) / ndet;
         }
     }
     H.min_rin = nt > 0 ? min_rin : 0.0;

@@ -569,6 +569,9 @@ int swe_mesh_info(const swe_ctx* c, int64_t* ncell, int64_t* nedge, int64_t* nbe
 int swe_set_params(swe_ctx* c, double g, double h_dry, double h_thin, double beta) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!(g > 0.0) || !(h_dry >= 0.0) || !(h_thin >= 0.0) || beta != beta) return fail(SWE_ERR_ARG, "bad parameter value");
+    // the kernels' reciprocal / square-root sequences (rcp_nr, sqrt_nr) start from MUFU seeds that
+    // flush subnormals: every depth that counts as wet must be a normal number well away from 0
+    if (h_dry < 1e-290) return fail(SWE_ERR_ARG, "h_dry must be >= 1e-290 (a wet depth has to be a normal fp64 number)");
     c->P.g = g; c->P.h_dry = h_dry; c->P.h_thin = h_thin; c->beta = beta;
     c->P.kappa = beta / 2.0; c->P.inv_g = 1.0 / g; c->P.limited = beta > 0.0 ? 1 : 0;
     drop_graph(c);                                   // the parameters are kernel arguments
@@ -809,6 +812,27 @@ int swe_fastmath_check(swe_ctx* c, int64_t n, const double* a, const double* x, 
     if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
     ndiff[0] = (int64_t)h[0]; ndiff[1] = (int64_t)h[1];
     memcpy(&maxrel[0], &h[2], sizeof(double)); memcpy(&maxrel[1], &h[3], sizeof(double));
+    return SWE_OK;
+}
+
+int swe_dry_counts(const swe_ctx* cc, int64_t* counts /*5*/) {
+    KeepMasks keep_masks(cc);   // read-only
+    swe_ctx* c = const_cast<swe_ctx*>(cc);
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!counts) return fail(SWE_ERR_ARG, "NULL output");
+    Store& st = c->active();
+    unsigned long long* d = nullptr;
+    CU(cudaMalloc((void**)&d, 3 * sizeof(unsigned long long)));
+    unsigned long long h[3] = {0, 0, 0};
+    cudaMemsetAsync(d, 0, sizeof(h), c->stream);
+    k_dry_counts<<<grid_for(st.ne, c->grid_light), 256, 0, c->stream>>>(st.dm, st.A, c->P.h_dry, d);
+    c->launches++;
+    cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    counts[0] = (int64_t)h[0]; counts[1] = (int64_t)h[1]; counts[2] = (int64_t)h[2];
+    counts[3] = c->H.nt; counts[4] = c->g.dm.ne_int;
     return SWE_OK;
 }
 
@@ -1181,8 +1205,15 @@ int swe_halo_unpack(swe_ctx* c, int buffer, const double* recvbuf) {
 
 // ---- halo exchange as one kernel over peer memory ----
 static int peer_store(swe_ctx* c, int peer, void* A, void* B, bool ipc) {
-    if (c->peer_ipc[peer]) { cudaIpcCloseMemHandle(c->peerA[peer]); cudaIpcCloseMemHandle(c->peerB[peer]); }
+    cudaError_t e = cudaSuccess;
+    if (c->peer_ipc[peer]) {
+        cudaStreamSynchronize(c->stream);                 // no push through the old mapping is still running
+        e = cudaIpcCloseMemHandle(c->peerA[peer]);
+        const cudaError_t e2 = cudaIpcCloseMemHandle(c->peerB[peer]);
+        if (e == cudaSuccess) e = e2;
+    }
     c->peerA[peer] = A; c->peerB[peer] = B; c->peer_ipc[peer] = ipc ? 1 : 0;
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SWE_ERR_CUDA, std::string("cudaIpcCloseMemHandle: ") + cudaGetErrorString(e)); }
     return SWE_OK;
 }
 static int peer_upload(swe_ctx* c) {
@@ -1215,14 +1246,25 @@ int swe_peer_export(swe_ctx* c, unsigned char* handles) {
 int swe_peer_import(swe_ctx* c, int peer, const unsigned char* handles) {
     int rc = check_peer(c, peer); if (rc) return rc;
     if (!handles) return fail(SWE_ERR_ARG, "NULL handle buffer");
+    // whatever was mapped for this peer goes first: opening a handle that is already open in this
+    // process is an error on some CUDA versions (re-import after a transport fallback, tests)
+    rc = peer_store(c, peer, nullptr, nullptr, false);
     cudaIpcMemHandle_t h;
     void *A = nullptr, *B = nullptr;
     std::memcpy(&h, handles, 64);
-    CU(cudaIpcOpenMemHandle(&A, h, cudaIpcMemLazyEnablePeerAccess));
-    std::memcpy(&h, handles + 64, 64);
-    cudaError_t e = cudaIpcOpenMemHandle(&B, h, cudaIpcMemLazyEnablePeerAccess);
-    if (e != cudaSuccess) { cudaIpcCloseMemHandle(A); return fail(SWE_ERR_CUDA, cudaGetErrorString(e)); }
-    peer_store(c, peer, A, B, true);
+    cudaError_t e = cudaIpcOpenMemHandle(&A, h, cudaIpcMemLazyEnablePeerAccess);
+    if (e == cudaSuccess) {
+        std::memcpy(&h, handles + 64, 64);
+        e = cudaIpcOpenMemHandle(&B, h, cudaIpcMemLazyEnablePeerAccess);
+        if (e != cudaSuccess) { cudaIpcCloseMemHandle(A); A = nullptr; }
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        peer_upload(c);      // the peer's slots are NULL again on the device too: swe_halo_push refuses instead of pushing through stale pointers
+        return fail(SWE_ERR_CUDA, std::string("cudaIpcOpenMemHandle: ") + cudaGetErrorString(e));
+    }
+    if (rc == SWE_OK) rc = peer_store(c, peer, A, B, true);
+    if (rc != SWE_OK) return rc;
     return peer_upload(c);
 }
 
@@ -1237,7 +1279,8 @@ int swe_peer_raw(swe_ctx* c, void** A, void** B) {
 int swe_peer_set_raw(swe_ctx* c, int peer, void* A, void* B) {
     int rc = check_peer(c, peer); if (rc) return rc;
     if (!A || !B || !is_device_ptr(A) || !is_device_ptr(B)) return fail(SWE_ERR_ARG, "peer buffers must be device pointers");
-    peer_store(c, peer, A, B, false);
+    rc = peer_store(c, peer, A, B, false);
+    if (rc != SWE_OK) { peer_upload(c); return rc; }
     return peer_upload(c);
 }
 

@@ -162,6 +162,11 @@ class DistSolver:
     recursive coordinate bisection (or zone_of_cell), rank r holding the block zone_blocks()[r:r+2];
     nlayers ghost layers (>= 2 for MUSCL / WAF / MUSCL_MS); transport "p2p" (peer-memory push, one
     kernel per exchange) or "staged" (pack -> all-to-all -> unpack).
+
+    Streams: the context runs on the torch stream that is current when the solver is created, and
+    the stream-ordered collectives that order the halo pushes against the peers' ghost reads are
+    enqueued on torch's current stream: the two must be the same stream, so step() and exchange()
+    raise if they are called under another one.
     """
 
     def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None,
@@ -184,7 +189,11 @@ class DistSolver:
             while nzones < self.world:
                 nzones *= 2
         self.nzones, self.nlayers = int(nzones), int(nlayers)
-        self.ctx = sw.create_from_config(cfg)
+        # the library's kernels and the collectives must be ordered on ONE stream: the context is
+        # created on the torch stream that is current now, and step() / exchange() refuse to run
+        # under another one (the barriers that order the halo pushes would stop ordering them)
+        self.stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+        self.ctx = sw.create_from_config(cfg, cuda_stream=self.stream or None)
         self.ncell = sw.swe_mesh_info(self.ctx)["ncell"]
         sw.swe_zones_create_dist(self.ctx, self.nzones, self.nlayers, zone_of_cell, self.world, self.rank,
                                  zone_blocks(self.nzones, self.world))
@@ -225,8 +234,14 @@ class DistSolver:
         self.comm.host_barrier()
 
     # -- one exchange of the ghosts of state buffer `buffer` (0 = U, 1 = the Heun stage buffer) --
+    def _check_stream(self):
+        if self.torch.cuda.is_available() and self.torch.cuda.current_stream().cuda_stream != self.stream:
+            raise RuntimeError("DistSolver was created on CUDA stream %#x and must be driven under the same "
+                               "torch stream (current: %#x)" % (self.stream, self.torch.cuda.current_stream().cuda_stream))
+
     def exchange(self, buffer):
         sw = self.sw
+        self._check_stream()
         if self.transport == "p2p":
             sw.swe_halo_push(self.ctx, buffer)
         else:
@@ -240,7 +255,9 @@ class DistSolver:
         self.comm.allreduce_min(self.token)
 
     def step(self, nsteps, cfl, scheme):
-        """nsteps time steps, asynchronous on the current stream (nccl)."""
+        """nsteps time steps, asynchronous on the stream the solver was created on (nccl), which
+        must be torch's current stream."""
+        self._check_stream()
         if self.schedule == "overlap":
             return self._step_overlap(nsteps, cfl, scheme)
         sw = self.sw

@@ -181,27 +181,29 @@ def test_config1_full():
 @pytest.mark.parametrize("scheme", ["waf", "muscl"])
 def test_config2_full(scheme):
     """configs[2]: ~1.0 M cells, lake at rest over rough bathymetry with dry bump tops, Manning
-    0.03, 1 000 steps: velocity <= 1e-12, mass conserved, masks identical; oracle parity over the
-    first 100 steps (the oracle needs minutes for 1 000) and GPU-only invariants to step 1 000."""
+    0.03, the stated 1 000 steps with the oracle running ALL of them beside the GPU (16 host cores:
+    15-35 s): per-step bar after step 1, run bar at steps 100 and 1 000, masks identical;
+    velocity <= 1e-12 and mass conserved on both sides."""
     cfg = config2()
     o, c = _pair(cfg)
     try:
         area = o.cell_geometry()["area"]
         m0 = float(np.sum(cfg["h"] * area))
         wet0 = cfg["h"] > 1e-6
-        o.step(1, 0.45, scheme)
-        sw.swe_step(c, 1, 0.45, scheme)
-        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c2 %s step 1" % scheme)
-        o.step(99, 0.45, scheme)
-        sw.swe_step(c, 99, 0.45, scheme)
-        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_RUN, what="c2 %s 100 steps" % scheme)
-        sw.swe_step(c, 900, 0.45, scheme)
-        h, hu, hv = sw.swe_get_state(c)
-        wet = h > 1e-6
-        assert np.array_equal(wet, wet0)
-        vel = np.sqrt(hu[wet] ** 2 + hv[wet] ** 2) / h[wet]
-        assert vel.max() <= 1e-12, vel.max()
-        assert abs(float(np.sum(h * area)) - m0) <= 1e-13 * m0
+        done = 0
+        for chunk in (1, 99, 900):
+            o.step(chunk, 0.45, scheme)
+            sw.swe_step(c, chunk, 0.45, scheme)
+            done += chunk
+            assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP if done == 1 else TOL_RUN,
+                          what="c2 %s after %d steps" % (scheme, done))
+        assert abs(sw.swe_get_time(c)[0] - o.step(0, 0.45, scheme)[0]) <= 1e-12 * sw.swe_get_time(c)[0]
+        for h, hu, hv in (sw.swe_get_state(c), o.get_state()):
+            wet = h > 1e-6
+            assert np.array_equal(wet, wet0)
+            vel = np.sqrt(hu[wet] ** 2 + hv[wet] ** 2) / h[wet]
+            assert vel.max() <= 1e-12, vel.max()
+            assert abs(float(np.sum(h * area)) - m0) <= 1e-13 * m0
     finally:
         sw.swe_mesh_destroy(c)
         o.close()
@@ -227,19 +229,28 @@ def test_config3_reduced_long_run():
 
 
 @pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9)])
-def test_config3_full_first_steps(scheme, cfl):
-    """configs[3] at full size (~13 M cells), in the launch configuration bench.py times: the
-    oracle advances 2 steps (it needs ~10 s per step), compared element by element."""
+def test_config3_full_stated_step_count(scheme, cfl):
+    """configs[3] at full size (13.1 M cells), in the launch configuration bench.py times, for the
+    stated 200 steps with the oracle running all of them beside the GPU (20 steps,
+    "all 200 if the OpenMP oracle needs < 10 min": it needs 40 s for HLLC, 130 s for MUSCL on the
+    box's 16 cores).  Free run from the initial state, compared element by element: per-step bar
+    after step 1, run bar after 2, 20, 100 and 200 steps, identical wet/dry masks throughout.
+    Measured (round 2): MUSCL 2e-15 after 200 steps; HLLC 2e-14 until step 190 and 4e-10 at step
+    200, where one wet/dry front decision falls on different steps on the two sides (DESIGN.md
+    section 3) -- inside the 1e-8 bar."""
     cfg = config3()
     o, c = _pair(cfg)
     try:
         assert o.nt > 12_000_000
-        o.step(1, cfl, scheme)
-        sw.swe_step(c, 1, cfl, scheme)
-        assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP, what="c3 %s step 1" % scheme)
-        o.step(1, cfl, scheme)
-        sw.swe_step(c, 1, cfl, scheme)
-        assert_parity(o.get_state(), sw.swe_get_state(c), 10 * TOL_STEP, what="c3 %s step 2" % scheme)
+        done = 0
+        for chunk in (1, 1, 18, 80, 100):
+            to, _ = o.step(chunk, cfl, scheme)
+            tg, _ = sw.swe_step(c, chunk, cfl, scheme)
+            done += chunk
+            tol = TOL_STEP if done == 1 else TOL_RUN
+            e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, done))
+            print("c3 full %s after %d steps: %s" % (scheme, done, e))
+            assert abs(tg - to) <= 1e-11 * to
     finally:
         sw.swe_mesh_destroy(c)
         o.close()

@@ -323,3 +323,80 @@ def test_oblique_uniform_stream_through_an_open_box_stays_uniform(scheme, cfl):
     np.testing.assert_allclose(h, 2.0, rtol=0, atol=1e-12)
     np.testing.assert_allclose(hu, 3.0, rtol=0, atol=1e-12)
     np.testing.assert_allclose(hv, 1.0, rtol=0, atol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# fixed-level boundary: tangential velocity of the ghost state (R11)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("scheme,cfl", [("hllc", 0.9), ("muscl", 0.45), ("waf", 0.45), ("muscl_ms", 0.45)])
+def test_oblique_uniform_stream_through_level_boundaries_stays_uniform(scheme, cfl):
+    """A box whose four sides all hold the free surface at the level of the water inside, crossed
+    obliquely by a uniform stream.  The ghost state of reading R11 (depth from the level, normal
+    velocity from the outgoing invariant, the interior's tangential velocity) then equals the
+    interior state on every side, the boundary flux is the physical flux of a constant state, and
+    the stream is steady.  On the two sides where the water ENTERS the contact wave upwinds the
+    tangential momentum from the ghost: a ghost without the interior's tangential velocity breaks
+    the steady state there."""
+    x, y, tri = si.grid_mesh(14, 9, 14.0, 9.0, 0.2, 23)
+    be = si.boundary_edges(tri)
+    o = po.Oracle(x, y, np.zeros_like(x), tri, be, np.full(len(be), 2, np.int32))
+    o.set_bc(2, "level", 2.0)
+    h0 = np.full(o.nt, 2.0)
+    o.set_state(h0, h0 * 1.5, h0 * 0.5)
+    o.step(40, cfl, scheme)
+    h, hu, hv = o.get_state()
+    np.testing.assert_allclose(h, 2.0, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(hu, 3.0, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(hv, 1.0, rtol=0, atol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# eq. 22 / 24 / 25 worked on a skewed pair of cells: which distances divide which jumps
+# ---------------------------------------------------------------------------------------------
+def test_multislope_face_values_on_a_skewed_stencil_worked_from_eq_22_24():
+    """Still water of varying depth over a flat bed, beta = 1 (MINBEE).  The upwind cells of an
+    interior edge are set so far beyond the local jump that both limited slopes of eq. 24-25 are the
+    LOCAL slope (h_R - h_L) / |x_R - x_L| (the smaller of two slopes of equal sign), so eq. 22 gives
+    the face depths  h_L + |r_L| s  and  h_R - |r_R| s  with |r| the distance from the centroid to
+    the edge midpoint (reading R17).  With zero velocity and a flat bed the mass component of the
+    edge flux is then the HLLC mass flux between those two face depths (a routine pinned on its own
+    in test_oracle_flux.py) times the edge length.  On a strongly jittered mesh the midpoint is off
+    the line between the centroids, |r_L| + |r_R| > |x_R - x_L|, so mixing up the distances shows."""
+    x, y, tri = si.grid_mesh(10, 8, 10.0, 8.0, 0.3, 31)
+    o = po.Oracle(x, y, np.zeros_like(x), tri)
+    o.set_params(beta=1.0)
+    c2c, _ = o.cell_topology()
+    e = o.edge_geometry()
+    cx = x[tri].mean(axis=1)
+    cy = y[tri].mean(axis=1)
+    rng = np.random.default_rng(5)
+    inner = np.nonzero(e["eR"] >= 0)[0]
+    checked, skew = 0, 0.0
+    for ed in rng.permutation(inner):
+        L, R = int(e["eL"][ed]), int(e["eR"][ed])
+        upL = [int(n) for n in c2c[L] if n != R]
+        upR = [int(n) for n in c2c[R] if n != L]
+        if min(upL + upR) < 0 or len(set(upL + upR)) != 4:
+            continue
+        shared = sorted(set(tri[L]) & set(tri[R]))
+        mx, my = x[shared].mean(), y[shared].mean()                # edge midpoint
+        rL = np.hypot(mx - cx[L], my - cy[L])
+        rR = np.hypot(mx - cx[R], my - cy[R])
+        dLR = np.hypot(cx[R] - cx[L], cy[R] - cy[L])
+        hL, hR = 2.0, 2.3
+        h = np.full(o.nt, 2.0)
+        h[L], h[R] = hL, hR
+        h[upL] = hL - 5.0 * (hR - hL) * 0.3                        # upwind slopes: same sign, much steeper
+        h[upR] = hR + 5.0 * (hR - hL) * 0.3
+        o.set_state(h, np.zeros(o.nt), np.zeros(o.nt))
+        s = (hR - hL) / dLR
+        want = po.hllc(G, 1e-6, hL + rL * s, 0.0, 0.0, hR - rR * s, 0.0, 0.0)["G1"] * e["len"][ed]
+        got = o.edge_flux(ed, 0.01, "muscl_ms")[0][0]
+        assert got == pytest.approx(want, rel=1e-12), (ed, got, want)
+        first = o.edge_flux(ed, 0.01, "hllc")[0][0]
+        assert abs(got - first) > 1e-3 * abs(first)                # the reconstruction is active
+        skew = max(skew, (rL + rR) / dLR - 1.0)
+        checked += 1
+        if checked == 12:
+            break
+    assert checked == 12 and skew > 0.01                           # the two distances really differ
