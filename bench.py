@@ -191,7 +191,7 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workload, fused=False):
+def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workload):
     """Per-kernel figures from the CUDA-event profile of the timed step loop (swe_get_profile)."""
     kern = {}
     tot_ms = sum(v[0] for v in prof.values())
@@ -209,11 +209,6 @@ def kernel_roofline(prof, steps, scheme, cells, step_ms, peak, peak_src, workloa
         algo = {"edge_flux": ALGO_BYTES["edge_flux_hllc"], "cell_update": ALGO_BYTES["cell_update_euler"]}
     else:
         algo = {"edge_flux": ALGO_BYTES["edge_flux_waf"], "cell_update": ALGO_BYTES["cell_update_euler"]}
-    if fused and "cell_update" not in kern:
-        # one pass does rows a3-a8: it is credited with the algorithmic bytes of BOTH passes it replaces
-        # ("if the build fuses passes it still reports against the fixed figure")
-        algo["flux_update_fused"] = algo.pop("edge_flux") + algo.pop("cell_update")
-        kern["flux_update_fused"] = kern.pop("edge_flux")
     for k in algo:
         if k in kern:
             kern[k]["algo_GBps"] = algo[k] * cells / (kern[k]["ms_per_launch"] * 1e-3) / 1e9
@@ -358,8 +353,6 @@ def main():
     ap.add_argument("--dry-masks", action="store_true",
                     help="swe_set_dry_masks on: leave the records of cells / edges without water alone (un-zoned mesh only)")
     ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--no-fused", action="store_true",
-                    help="Heun schemes: the three-kernel pipeline with the flux buffer instead of the fused flux + update pass")
     ap.add_argument("--reps", type=int, default=5,
                     help="the timed region of K steps is run this many times; value = the median (BASELINE.md section 4)")
     ap.add_argument("--no-all-wet", action="store_true",
@@ -398,8 +391,6 @@ def main():
         sw.swe_zones_create(ctx, args.zones, args.layers)
     if args.dry_masks:
         sw.swe_set_dry_masks(ctx, True)
-    sw.swe_set_fused(ctx, not args.no_fused)
-    fused = (not args.no_fused) and not args.dry_masks and args.scheme in ("muscl", "muscl_ms")
 
     # ---- device-resident throughput: warm-up, then exactly K timed steps, `reps` times over ----
     sw.swe_step(ctx, args.warmup, cfl, args.scheme)
@@ -432,7 +423,7 @@ def main():
     clocks = clk.stop()
     peak, peak_src = hbm_peak()
     roofline = kernel_roofline(prof, args.steps, args.scheme, nt, ms / args.steps, peak, peak_src,
-                               args.workload + ("+masks" if args.dry_masks and args.zones == 0 else ""), fused)
+                               args.workload + ("+masks" if args.dry_masks and args.zones == 0 else ""))
     roofline["dry_state"] = {
         "cells_not_wet_frac": dry["cells_not_wet"] / dry["cells"], "cells_empty_frac": dry["cells_empty"] / dry["cells"],
         "edges_between_empty_cells_frac": dry["edges_between_empty_cells"] / max(1, dry["interior_edges"]),
@@ -455,7 +446,7 @@ def main():
         sw.swe_step(ctx, args.steps, cfl, args.scheme)
         wprof = sw.swe_get_profile(ctx)
         sw.swe_set_profile(ctx, False)
-        wr = kernel_roofline(wprof, args.steps, args.scheme, nt, wms / args.steps, peak, peak_src, "c3w", fused)
+        wr = kernel_roofline(wprof, args.steps, args.scheme, nt, wms / args.steps, peak, peak_src, "c3w")
         roofline["all_wet"] = {
             "workload": "the same mesh and bed flooded to a flat surface at 18 m (swe_inputs.flooded), %d warm-up steps, "
                         "median of 3 x %d timed steps" % (args.warmup, args.steps),
@@ -520,10 +511,7 @@ def main():
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
                        "zones": args.zones, "ghost_layers": args.layers if args.zones else 0,
                        "renumber": args.renumber,
-                       "dry_masks": args.dry_masks and args.zones == 0,
-                       "pipeline": "per stage: gradient + limiter pass, then ONE fused edge-flux + cell-update pass (no flux buffer)"
-                       if fused else "per stage: gradient pass (Heun schemes), edge-flux pass (flux buffer), cell-update pass",
-                       "paper_context": PAPER_CONTEXT[args.scheme]},
+                       "dry_masks": args.dry_masks and args.zones == 0, "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
             "gpu_launches": int(launches_per_rep), "clocks": clocks,
             "reps": {"n": len(rep_ms), "ms_per_step": [m / args.steps for m in rep_ms],

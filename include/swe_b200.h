@@ -102,14 +102,6 @@ int swe_step(swe_ctx* ctx, int nsteps, double cfl, int scheme, double* t_out, do
  * ~1 M cells the step is launch-bound).  on = 0 launches the kernels one by one (default: on).  The
  * results are identical either way. */
 int swe_set_graphs(swe_ctx* ctx, int on);
-/* Heun schemes (SWE_MUSCL, SWE_MUSCL_MS) in swe_step: on (default) = a stage is the cell pass of
- * the gradients / slope records followed by ONE fused pass in which every owned cell evaluates the
- * fluxes of its three edges (rows a3-a7) and updates itself (row a8), with no flux buffer in
- * between; off = the three-kernel pipeline gradient -> edge flux (flux buffer) -> cell update, which
- * the Euler schemes (in-place update), the dry-record masks and the distributed stages always
- * use.  Both evaluate an edge with the same device function in the same L | R orientation and sum
- * in side order: results are bit-identical (tests/test_gpu_fused.py).  Errors: SWE_ERR_ARG. */
-int swe_set_fused(swe_ctx* ctx, int on);
 
 /* Cells without water are not worked on (wet/dry treatment of SURVEY.md section 8(c), A.3.5 /
  * A.6: a cell whose record is (0, 0, 0, z) has zero gradients, and an interior edge between two

@@ -38,7 +38,6 @@ SIGNATURES = {
     "swe_set_time": (C.c_int, [_vp, C.c_double]),
     "swe_step": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, _dp, _dp]),
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
-    "swe_set_fused": (C.c_int, [_vp, C.c_int]),
     "swe_set_dry_masks": (C.c_int, [_vp, C.c_int]),
     "swe_fp64_peak": (C.c_int, [_vp, _dp]),
     "swe_dry_counts": (C.c_int, [_vp, _i64p]),
@@ -229,10 +228,6 @@ def swe_fp64_peak(ctx):
 
 def swe_set_dry_masks(ctx, on):
     _check(lib().swe_set_dry_masks(ctx, 1 if on else 0))
-
-
-def swe_set_fused(ctx, on):
-    _check(lib().swe_set_fused(ctx, 1 if on else 0))
 
 
 def swe_set_graphs(ctx, on):
@@ -439,7 +434,7 @@ def create_from_config(cfg, renumber=SWE_RENUM_HILBERT, cuda_stream=None):
 
 
 # ---- host-only inspection (no GPU) ----------------------------------------------------------
-_HOST_DTYPES = {"eside": np.uint8, "tri": np.int32, "cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": np.int32, "btag": np.int32,
+_HOST_DTYPES = {"eside": np.uint8, "cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": np.int32, "btag": np.int32,
                 "user_cell": np.int32, "zone_of": np.int32, "send_idx": np.int32, "recv_idx": np.int32,
                 "src_of_cell": np.int32, "link_src": np.int32, "link_dst": np.int32, "tags": np.int32,
                 "zone_rank": np.int32, "rsend_idx": np.int32, "rsend_dst": np.int32, "rsend_peer": np.int32,

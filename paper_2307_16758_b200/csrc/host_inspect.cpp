@@ -46,8 +46,6 @@ int64_t mesh_get(const MeshArrays& M, const std::string& n, void* out, int64_t c
     if (n == "edlr") return copy_out(M.edlr, out, cap);
     if (n == "eside") return copy_out(M.eside, out, cap);
     if (n == "ernorm") return copy_out(M.ernorm, out, cap);
-    if (n == "tri") return copy_out(M.tri, out, cap);
-    if (n == "cxy") return copy_out(M.cxy, out, cap);
     return -2;
 }
 }  // namespace
@@ -104,7 +102,6 @@ int64_t swe_host_get(void* hh, const char* name, void* out, int64_t cap_bytes) {
     if (n == "user_cell") return copy_out(h->H.user_cell, out, cap_bytes);
     if (n == "cx") return copy_out(h->H.cx, out, cap_bytes);
     if (n == "cy") return copy_out(h->H.cy, out, cap_bytes);
-    if (n == "vxy") return copy_out(h->H.vxy, out, cap_bytes);
     if (n == "tags") return copy_out(h->H.tags, out, cap_bytes);
     if (n == "tag_width") return copy_out(h->H.tag_width, out, cap_bytes);
     if (n.rfind("z:", 0) == 0) {

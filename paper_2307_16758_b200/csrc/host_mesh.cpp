@@ -274,28 +274,6 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         M.err[2 * d] = rrx[e]; M.err[2 * d + 1] = rry[e];
         if (d >= M.ne_int) M.btag[d - M.ne_int] = utag[e];
     }
-    // vertices renumbered by first touch along the device cell order; per cell its three vertices
-    // (oriented as in A.1.1) and its centroid
-    {
-        std::vector<int32_t> vnew(nv, -1);
-        int32_t next = 0;
-        M.tri.assign(4 * (size_t)nt, 0);
-        M.cxy.resize(2 * (size_t)nt);
-        for (int64_t i = 0; i < nt; ++i) {
-            const int64_t u = cell_user[i];
-            for (int k = 0; k < 3; ++k) {
-                const int32_t v = tri[3 * u + k];
-                if (vnew[v] < 0) vnew[v] = next++;
-                M.tri[4 * i + k] = vnew[v];
-            }
-            M.cxy[2 * i] = ucx[u]; M.cxy[2 * i + 1] = ucy[u];
-        }
-        H.vxy.assign(2 * (size_t)nv, 0.0);
-        for (int64_t v = 0; v < nv; ++v) {
-            if (vnew[v] < 0) vnew[v] = next++;            // a vertex no triangle uses
-            H.vxy[2 * (size_t)vnew[v]] = x[v]; H.vxy[2 * (size_t)vnew[v] + 1] = y[v];
-        }
-    }
     double min_rin = 1e300;
     for (int64_t i = 0; i < nt; ++i) {
         int64_t u = cell_user[i];
@@ -570,8 +548,6 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne); M.edlr.resize(M.ne);
     M.eside.resize(M.ne); M.ernorm.resize(2 * M.ne);
     M.dupw.assign(4 * (size_t)ncz, 0.0);
-    M.tri.assign(4 * (size_t)ncz, 0);
-    M.cxy.resize(2 * (size_t)ncz);
     M.btag.assign(M.ne - M.ne_int, -1);
     std::vector<int32_t> eloc(G.ne, -1);
     for (int zi = 0; zi < nz; ++zi) {
@@ -602,8 +578,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             M.cell_user[c] = G.cell_user[g];
             Z.src_of_cell[c] = (int32_t)g;
             M.zc[c] = G.zc[g]; M.area[c] = G.area[g]; M.rin[c] = G.rin[g];
-            for (int k = 0; k < 3; ++k) { M.dupw[4 * c + k] = G.dupw[4 * g + k]; M.tri[4 * c + k] = G.tri[4 * g + k]; }
-            M.cxy[2 * c] = G.cxy[2 * g]; M.cxy[2 * c + 1] = G.cxy[2 * g + 1];
+            for (int k = 0; k < 3; ++k) M.dupw[4 * c + k] = G.dupw[4 * g + k];
             for (int k = 0; k < 3; ++k) {
                 M.w[k][2 * c] = G.w[k][2 * g]; M.w[k][2 * c + 1] = G.w[k][2 * g + 1];
                 M.r[k][2 * c] = G.r[k][2 * g]; M.r[k][2 * c + 1] = G.r[k][2 * g + 1];

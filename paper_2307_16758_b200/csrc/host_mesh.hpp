@@ -25,10 +25,6 @@ struct MeshArrays {
     std::vector<double> w[3];                // 2*nc each: least-squares weights (wx,wy) of side k
     std::vector<double> r[3];                // 2*nc each: r_{i,k} = m_e - c_i
     std::vector<double> dupw;                // 4*nc: |x_i - x_upw| for side 0,1,2 (multislope MUSCL), pad
-    std::vector<int32_t> tri;                // 4*nc: the cell's vertices v0, v1, v2 (counter-clockwise; side k joins
-                                             //       v_k -> v_k+1) as ids into HostMesh::vxy, pad
-    std::vector<double> cxy;                 // 2*nc: centroid (the gradient kernel derives r_k and the LSQ weights
-                                             //       from vertices and centroids instead of streaming them)
     // per edge
     std::vector<int32_t> elr;                // 2*ne: L cell, R cell (-1 on the boundary)
     std::vector<double> en;                  // 2*ne: unit normal, outward of L
@@ -82,8 +78,6 @@ struct HostMesh {
     double min_rin = 0.0;
     std::vector<int32_t> user_cell;          // user id -> device id
     std::vector<double> cx, cy;              // centroids, device numbering (zone builder)
-    std::vector<double> vxy;                 // 2*nv: vertex coordinates, vertices renumbered in the order the
-                                             //       cells (device numbering) first touch them (gather locality)
     MeshArrays m;                            // un-zoned mesh, device numbering
     std::vector<int32_t> tags;               // distinct user tags
     std::vector<double> tag_width;           // sum of edge lengths per tag

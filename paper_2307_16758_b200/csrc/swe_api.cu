@@ -118,9 +118,6 @@ struct swe_ctx {
     bool mk_on = false;                // set while swe_step enqueues its stages
     bool graph_masks = false;
     bool use_graphs = true;
-    bool fused = false;                // Heun schemes: flux + update in one cell pass, no flux buffer (swe_set_fused)
-    bool graph_fused = false;
-    int grid_fused[4] = {148 * 5, 148 * 5, 148 * 5, 148 * 5};
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t step_exec = nullptr;
     int graph_scheme = -1; double graph_cfl = 0.0; bool graph_zoned = false;
@@ -196,28 +193,11 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.upload(&area, M.area.data(), (size_t)M.nc, s));
     CU(st.upload(&rin, M.rin.data(), (size_t)M.nc, s));
     d.c2c = c2c; d.c2e = c2e; d.zc = zc; d.area = area; d.rin = rin;
-#if SWE_GRAD_ONFLY
-    for (int k = 0; k < 3; ++k) { d.w[k] = nullptr; d.r[k] = nullptr; }      // derived in the kernel (stencil_geom)
-#else
     for (int k = 0; k < 3; ++k) {
         double2 *w, *r;
         CU(st.upload(&w, M.w[k].data(), (size_t)M.nc, s));
         CU(st.upload(&r, M.r[k].data(), (size_t)M.nc, s));
         d.w[k] = w; d.r[k] = r;
-    }
-#endif
-    {
-        int4* tri; double2* cxy;
-        CU(st.upload(&tri, M.tri.data(), (size_t)M.nc, s));
-        CU(st.upload(&cxy, M.cxy.data(), (size_t)M.nc, s));
-        d.tri = tri; d.cxy = cxy;
-        if (&st == &c->g) {                          // one vertex array serves both stores
-            double2* vxy;
-            CU(st.upload(&vxy, c->H.vxy.data(), (size_t)c->H.nv, s));
-            d.vxy = vxy;
-        } else {
-            d.vxy = c->g.dm.vxy;
-        }
     }
     int2* elr; double2 *en, *erl, *err; double *elen, *edx;
     CU(st.upload(&elr, M.elr.data(), (size_t)M.ne, s));
@@ -449,35 +429,11 @@ void run_exchange_grad(swe_ctx* c) {
     c->halo_bytes += count * (4 + 64 + 64 + 4 + 64 + 64);
 }
 
-// Heun schemes, whole store: edge fluxes and cell update in one cell pass (k_cell_flux_update)
-void run_fused(swe_ctx* c, Store& st, const double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
-    launch(c, KIND_FLUX, [&] {
-        const int gr = grid_for(st.nc, c->grid_fused[scheme], SWE_FUSED_THREADS);
-#define SWE_FUSED_LAUNCH(SC, MO, FU) k_cell_flux_update<SC, MO, FU><<<gr, SWE_FUSED_THREADS, 0, c->stream>>>(st.dm, Uin, U0, Uout, st.grad, c->P, c->d_S, 0)
-        if (scheme == K_MUSCL) {
-            if (mode == 0 && !fuse) SWE_FUSED_LAUNCH(K_MUSCL, 0, false);
-            else if (mode == 0) SWE_FUSED_LAUNCH(K_MUSCL, 0, true);
-            else if (!fuse) SWE_FUSED_LAUNCH(K_MUSCL, 1, false);
-            else SWE_FUSED_LAUNCH(K_MUSCL, 1, true);
-        } else {
-            if (mode == 0 && !fuse) SWE_FUSED_LAUNCH(K_MUSCL_MS, 0, false);
-            else if (mode == 0) SWE_FUSED_LAUNCH(K_MUSCL_MS, 0, true);
-            else if (!fuse) SWE_FUSED_LAUNCH(K_MUSCL_MS, 1, false);
-            else SWE_FUSED_LAUNCH(K_MUSCL_MS, 1, true);
-        }
-#undef SWE_FUSED_LAUNCH
-    });
-}
-bool stage_is_fused(const swe_ctx* c, int scheme, const double4* Uin, const double4* Uout) {
-    return c->fused && !c->mk_on && (scheme == K_MUSCL || scheme == K_MUSCL_MS) && Uin != Uout;
-}
-
 // one Euler stage on the active store: [exchange] -> [grad (-> exchange grad)] -> flux -> update
 void run_stage(swe_ctx* c, Store& st, double4* Uin, const double4* U0, double4* Uout, int scheme, int mode, bool fuse) {
     if (c->has_zones) run_exchange_state(c, Uin, 0, c->nsend, true, true);
     run_grad(c, st, Uin, scheme);
     if (scheme == K_MUSCL && c->has_zones && c->Z.nlayers == 1) run_exchange_grad(c);
-    if (stage_is_fused(c, scheme, Uin, Uout)) { run_fused(c, st, Uin, U0, Uout, scheme, mode, fuse); return; }
     run_flux(c, st, Uin, scheme);
     run_update(c, st, Uin, U0, Uout, mode, fuse);
 }
@@ -559,8 +515,6 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS, false>, 2, SWE_FLUX_THREADS);
     c->grid_upd = occ((const void*)k_cell_update<1, true, false>, 4);
     c->grid_ms = occ((const void*)k_ms_slopes, 5, 128);
-    c->grid_fused[K_MUSCL] = occ((const void*)k_cell_flux_update<K_MUSCL, 1, true>, 4, SWE_FUSED_THREADS);
-    c->grid_fused[K_MUSCL_MS] = occ((const void*)k_cell_flux_update<K_MUSCL_MS, 1, true>, 4, SWE_FUSED_THREADS);
     int rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
         cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
@@ -764,7 +718,7 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
     if (c->use_graphs && !c->profile && nsteps >= 2) {
         // capture one step (same kernels, same order, same arguments) and replay it
         if (!c->step_exec || c->graph_scheme != scheme || c->graph_cfl != cfl || c->graph_zoned != c->has_zones ||
-            c->graph_masks != c->mk_on || c->graph_fused != c->fused) {
+            c->graph_masks != c->mk_on) {
             drop_graph(c);
             if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
             const int64_t l0 = c->launches, h0 = c->halo_bytes;
@@ -782,7 +736,7 @@ int swe_step(swe_ctx* c, int nsteps, double cfl, int scheme, double* t_out, doub
             if (e == cudaSuccess) e = cudaGraphInstantiate(&c->step_exec, graph, 0);
             if (graph) cudaGraphDestroy(graph);
             if (e != cudaSuccess) { c->step_exec = nullptr; return fail(SWE_ERR_CUDA, std::string("step graph: ") + cudaGetErrorString(e)); }
-            c->graph_scheme = scheme; c->graph_cfl = cfl; c->graph_zoned = c->has_zones; c->graph_masks = c->mk_on; c->graph_fused = c->fused;
+            c->graph_scheme = scheme; c->graph_cfl = cfl; c->graph_zoned = c->has_zones; c->graph_masks = c->mk_on;
         }
         for (; s0 < nsteps; ++s0) {
             CU(cudaGraphLaunch(c->step_exec, c->stream));
@@ -885,12 +839,6 @@ int swe_dry_counts(const swe_ctx* cc, int64_t* counts /*5*/) {
 int swe_set_dry_masks(swe_ctx* c, int on) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     c->dry_masks = on != 0;
-    return SWE_OK;
-}
-
-int swe_set_fused(swe_ctx* c, int on) {
-    if (check_ctx(c)) return SWE_ERR_ARG;
-    c->fused = on != 0;
     return SWE_OK;
 }
 
