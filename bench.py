@@ -257,7 +257,7 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
     import paper_2307_16758_b200 as sw
 
     S = swdist.DistSolver(cfg, nzones=args.zones if args.zones > 0 else None, nlayers=args.layers,
-                          transport=args.transport, schedule=args.schedule)
+                          transport=args.transport, schedule=args.schedule, graphs=not args.no_dist_graph)
     nt = S.ncell
     info = sw.swe_mesh_info(S.ctx)
     owned = sum(sw.swe_zone_describe_counts(S.ctx, z)[0] for z in range(*swdist.shard_units(S.nzones, rank, world)))
@@ -281,10 +281,14 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
     halo = swdist.reduce_sum(float(l1["halo_bytes"] - l0["halo_bytes"])) / args.steps
 
     # per-kernel CUDA events on this rank's launches (rank 0 reports its own share of the mesh)
-    sw.swe_set_profile(S.ctx, True)
+    host_us = S.host_us_per_step                   # host time per step of the timed call (enqueue only)
+    replays = S.graph_replays
+    S.set_profile(True)
     S.step(args.steps, cfl, args.scheme)
     prof = sw.swe_get_profile(S.ctx)
-    sw.swe_set_profile(S.ctx, False)
+    S.set_profile(False)
+    # exposed collective time: the step's device time minus this rank's kernels (events around every launch)
+    kern_ms = sum(v[0] for v in prof.values()) / args.steps
     clocks = clk.stop()
     peak, peak_src = hbm_peak()
     roofline = kernel_roofline(prof, args.steps, args.scheme, owned, ms / args.steps, peak, peak_src, args.workload)
@@ -325,6 +329,9 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
                                       "schedule %s, all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport,
                                                                               S.schedule),
                        "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo,
+                       "step_as_cuda_graph": bool(replays), "host_us_per_step": host_us,
+                       "rank0_kernel_ms_per_step": kern_ms,
+                       "rank0_not_in_kernels_ms_per_step": max(0.0, ms / args.steps - kern_ms),
                        "paper_context": PAPER_CONTEXT[args.scheme]},
             "roofline": roofline, "e2e": e2e, "cpu_baseline": None,
             "gpu_launches": int(launches), "clocks": clocks,
@@ -348,6 +355,8 @@ def main():
     ap.add_argument("--schedule", default="overlap", choices=["overlap", "plain"])
     ap.add_argument("--force-dist", action="store_true",
                     help="run the distributed arm (DistSolver, zones over ranks) even with a single rank")
+    ap.add_argument("--no-dist-graph", action="store_true",
+                    help="distributed arm: enqueue every step call by call instead of replaying it as one CUDA graph")
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of one split mesh")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dry-masks", action="store_true",

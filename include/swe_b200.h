@@ -233,6 +233,12 @@ int swe_side_fluxes(swe_ctx* ctx, double dt, int scheme, double* out);
 int swe_euler_stage(swe_ctx* ctx, double dt, int scheme, double* h1, double* hu1, double* hv1);
 /* counters: steps taken, kernels launched by this context so far, bytes moved by pack+unpack. */
 int swe_get_stats(const swe_ctx* ctx, int64_t* steps, int64_t* kernel_launches, int64_t* halo_bytes);
+/* For a caller that captures a sequence of this context's calls into a CUDA graph of its own and
+ * replays it (paper_2307_16758_b200/dist.py does so for the distributed step, collectives included):
+ * adds the steps, kernel launches and halo bytes of the replays to the counters of swe_get_stats
+ * (the library only sees the calls made during the capture).  Arguments may be negative (to take
+ * the recorded-but-not-run capture pass out again).  Errors: SWE_ERR_ARG. */
+int swe_account_replays(swe_ctx* ctx, int64_t steps, int64_t kernel_launches, int64_t halo_bytes);
 /* time the hot path with CUDA events on the context's stream: runs swe_step(nsteps,...) between
  * two events and returns the elapsed milliseconds (synchronises). */
 int swe_step_timed(swe_ctx* ctx, int nsteps, double cfl, int scheme, float* ms_out);

@@ -71,6 +71,7 @@ SIGNATURES = {
     "swe_side_fluxes": (C.c_int, [_vp, C.c_double, C.c_int, _vp]),
     "swe_euler_stage": (C.c_int, [_vp, C.c_double, C.c_int, _vp, _vp, _vp]),
     "swe_get_stats": (C.c_int, [_vp, _i64p, _i64p, _i64p]),
+    "swe_account_replays": (C.c_int, [_vp, C.c_int64, C.c_int64, C.c_int64]),
     "swe_step_timed": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, C.POINTER(C.c_float)]),
     "swe_kernel_timed": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float)]),
     "swe_set_profile": (C.c_int, [_vp, C.c_int]),
@@ -384,6 +385,10 @@ def swe_euler_stage(ctx, dt, scheme):
     h, hu, hv = np.empty(n), np.empty(n), np.empty(n)
     _check(lib().swe_euler_stage(ctx, float(dt), _scheme(scheme), _ptr(h), _ptr(hu), _ptr(hv)))
     return h, hu, hv
+
+
+def swe_account_replays(ctx, steps, kernel_launches, halo_bytes):
+    _check(lib().swe_account_replays(ctx, int(steps), int(kernel_launches), int(halo_bytes)))
 
 
 def swe_get_stats(ctx):

@@ -1002,6 +1002,13 @@ int swe_get_stats(const swe_ctx* c, int64_t* steps, int64_t* kernel_launches, in
     return SWE_OK;
 }
 
+int swe_account_replays(swe_ctx* c, int64_t steps, int64_t kernel_launches, int64_t halo_bytes) {
+    KeepMasks keep_masks(c);
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    c->steps += steps; c->launches += kernel_launches; c->halo_bytes += halo_bytes;
+    return SWE_OK;
+}
+
 // ---- zones ----
 // Row f4: the ghost layers of all zones on the device (swe_zone_kernels.cuh).  zone_of: per cell of
 // the un-zoned mesh, device numbering.  Returns the sorted keys build_zones consumes.

@@ -170,7 +170,7 @@ class DistSolver:
     """
 
     def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None,
-                 schedule="overlap"):
+                 schedule="overlap", graphs=True):
         import torch
         from . import binding as sw
         self.sw, self.torch = sw, torch
@@ -182,18 +182,26 @@ class DistSolver:
         if schedule not in ("plain", "overlap"):
             raise ValueError("schedule must be 'plain' or 'overlap'")
         self.schedule = schedule
-        self._bar = self._minwork = None
         self._primed = False
         if nzones is None:
             nzones = 1
             while nzones < self.world:
                 nzones *= 2
         self.nzones, self.nlayers = int(nzones), int(nlayers)
-        # the library's kernels and the collectives must be ordered on ONE stream: the context is
-        # created on the torch stream that is current now, and step() / exchange() refuse to run
-        # under another one (the barriers that order the halo pushes would stop ordering them)
-        self.stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
-        self.ctx = sw.create_from_config(cfg, cuda_stream=self.stream or None)
+        # the library's kernels and the collectives must be ordered on ONE stream: the solver owns
+        # a stream, creates the context on it and issues every library call and every collective
+        # under it; step() / exchange() / set_state() order that stream behind the caller's current
+        # stream on entry and the caller's stream behind it on exit
+        self.tstream = torch.cuda.Stream() if torch.cuda.is_available() else None
+        self.stream = self.tstream.cuda_stream if self.tstream is not None else 0
+        self.graphs = bool(graphs)
+        self._graph = {}                # (scheme, cfl, body) -> (CUDAGraph, launches, halo bytes, steps) of one step
+        self.graph_replays = 0
+        self.host_us_per_step = None    # host time of the last step() call per step (enqueue only)
+        self._flux_done = None
+        self.profile = False
+        with self._on_stream():
+            self.ctx = sw.create_from_config(cfg, cuda_stream=self.stream or None)
         self.ncell = sw.swe_mesh_info(self.ctx)["ncell"]
         sw.swe_zones_create_dist(self.ctx, self.nzones, self.nlayers, zone_of_cell, self.world, self.rank,
                                  zone_blocks(self.nzones, self.world))
@@ -234,14 +242,34 @@ class DistSolver:
         self.comm.host_barrier()
 
     # -- one exchange of the ghosts of state buffer `buffer` (0 = U, 1 = the Heun stage buffer) --
-    def _check_stream(self):
-        if self.torch.cuda.is_available() and self.torch.cuda.current_stream().cuda_stream != self.stream:
-            raise RuntimeError("DistSolver was created on CUDA stream %#x and must be driven under the same "
-                               "torch stream (current: %#x)" % (self.stream, self.torch.cuda.current_stream().cuda_stream))
+    def _on_stream(self):
+        """Context manager: run under the solver's stream, ordered behind the caller's current
+        stream on entry; the caller's stream is ordered behind the solver's on exit."""
+        import contextlib
+        torch = self.torch
 
+        @contextlib.contextmanager
+        def cm():
+            if self.tstream is None:
+                yield
+                return
+            cur = torch.cuda.current_stream()
+            if cur.cuda_stream == self.tstream.cuda_stream:      # already inside (nested call)
+                yield
+                return
+            self.tstream.wait_stream(cur)
+            with torch.cuda.stream(self.tstream):
+                yield
+            cur.wait_stream(self.tstream)
+        return cm()
+
+    # -- one exchange of the ghosts of state buffer `buffer` (0 = U, 1 = the Heun stage buffer) --
     def exchange(self, buffer):
+        with self._on_stream():
+            self._exchange(buffer)
+
+    def _exchange(self, buffer):
         sw = self.sw
-        self._check_stream()
         if self.transport == "p2p":
             sw.swe_halo_push(self.ctx, buffer)
         else:
@@ -252,116 +280,203 @@ class DistSolver:
 
     def barrier_stream(self):
         """Stream-ordered barrier: nobody's stream passes it before everybody's reached it."""
-        self.comm.allreduce_min(self.token)
+        with self._on_stream():
+            self.comm.allreduce_min(self.token)
 
-    def step(self, nsteps, cfl, scheme):
-        """nsteps time steps, asynchronous on the stream the solver was created on (nccl), which
-        must be torch's current stream."""
-        self._check_stream()
-        if self.schedule == "overlap":
-            return self._step_overlap(nsteps, cfl, scheme)
-        sw = self.sw
-        sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
-        heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
-        p2p = self.transport == "p2p"
-        for _ in range(int(nsteps)):
-            self.exchange(0)
-            sw.swe_dist_local_min(self.ctx, self.minbuf)
-            self.comm.allreduce_min(self.minbuf)       # dt; with p2p also: every push of buffer 0 has landed
-            sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
-            sw.swe_dist_stage(self.ctx, sch, 0)
-            if heun:
-                self.exchange(1)
-                if p2p:
-                    self.barrier_stream()              # every push of buffer 1 has landed
-                sw.swe_dist_stage(self.ctx, sch, 1)
-            elif p2p:
-                self.barrier_stream()                  # everybody has read its ghosts of buffer 0
+    def _exchange_async(self, buffer):
+        self._exchange(buffer)
+        return self.comm.allreduce_min_async(self.token) if self.transport == "p2p" else None
 
-    # -- overlap schedule (scope row f2; PAPER.md:462 "high overlap") ------------------------------
-    # Every stage updates the cells on the send lists first, exchanges them, starts the barrier
-    # asynchronously and updates the rest of the domain while the collective is in flight; the
-    # all-reduce of dt likewise runs behind the next gradient / flux pass (dt is first needed by
-    # the update; WAF needs it in the flux).  Hazards (buffer b = 0: U, 1: the Heun stage buffer):
-    #   * a rank reads its ghosts of b only after wait(barrier) of the exchange of b;
-    #   * an exchange of b is issued after a wait() on a collective that every rank started after
+    # -- the step ---------------------------------------------------------------------------------
+    # Invariant between steps ("primed"): the ghosts of buffer 0 are current on every rank and
+    # minbuf holds the all-reduced minimum of R_i / lambda_i of U^n -- both collectives have been
+    # waited for on the stream (a stream wait: the host never blocks).
+    #
+    # schedule "plain": the serial order  flux, update, exchange, barrier  per stage.
+    # schedule "overlap" (scope row f2; PAPER.md:462 "high overlap"): every stage updates the cells
+    # on the send lists first, exchanges them, starts the barrier asynchronously and updates the
+    # rest of the domain while the collective is in flight.  The all-reduce of dt is hidden too: for
+    # every scheme but WAF the body is ROTATED -- it starts behind the gradient / flux pass of its
+    # first stage and ends with that pass of the NEXT step, which runs while the all-reduce of the
+    # minimum is in flight (dt is first needed by the update; WAF needs it in the flux and keeps the
+    # unrotated order).  `_flux_done` remembers for which scheme that pass has been enqueued.
+    # Hazards (buffer b = 0: U, 1: the Heun stage buffer):
+    #   * a rank reads its ghosts of b only behind wait(barrier) of the exchange of b;
+    #   * an exchange of b is issued behind a wait() on a collective that every rank started after
     #     its last flux pass over b, so nobody's ghosts are overwritten while still being read.
     #     Heun: the barrier of the other buffer's exchange is that collective.  Euler schemes have
     #     one buffer: they start one more barrier right after the flux pass and wait for it before
     #     the exchange.
-    def _exchange_async(self, buffer):
-        self.exchange(buffer)
-        return self.comm.allreduce_min_async(self.token) if self.transport == "p2p" else None
-
-    def _step_overlap(self, nsteps, cfl, scheme):
+    # With the nccl backend one step (same kernels, same collectives, same order; dt lives in
+    # device memory) is captured ONCE as a CUDA graph per (scheme, cfl) and replayed: the host then
+    # spends one graph launch per step instead of ~15 C calls and 3 torch.distributed calls.
+    def _prime(self):
         sw, comm = self.sw, self.comm
-        sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
+        if self._primed:
+            return
+        bar = self._exchange_async(0)
+        sw.swe_dist_local_min(self.ctx, self.minbuf)
+        mw = comm.allreduce_min_async(self.minbuf)
+        comm.wait(bar)
+        comm.wait(mw)
+        self._primed = True
+        self._flux_done = None
+
+    def _body_plain(self, sch, cfl):
+        sw = self.sw
+        heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
+        p2p = self.transport == "p2p"
+        sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+        sw.swe_dist_stage(self.ctx, sch, 0)
+        if heun:
+            self._exchange(1)
+            if p2p:
+                self.comm.allreduce_min(self.token)    # every push of buffer 1 has landed
+            sw.swe_dist_stage(self.ctx, sch, 1)
+        elif p2p:
+            self.comm.allreduce_min(self.token)        # everybody has read its ghosts of buffer 0
+        self._exchange(0)
+        sw.swe_dist_local_min(self.ctx, self.minbuf)
+        self.comm.allreduce_min(self.minbuf)           # dt; with p2p also: every push of buffer 0 has landed
+
+    def _body_overlap(self, sch, cfl):
+        sw, comm = self.sw, self.comm
         heun = sch in (sw.SWE_MUSCL, sw.SWE_MUSCL_MS)
         waf = sch == sw.SWE_WAF
         p2p = self.transport == "p2p"
-        for _ in range(int(nsteps)):
-            if not self._primed:                       # first step after set-up / set_state
-                self._bar = self._exchange_async(0)
-                sw.swe_dist_local_min(self.ctx, self.minbuf)
-                self._minwork = comm.allreduce_min_async(self.minbuf)
-                self._primed = True
-            comm.wait(self._bar)                       # ghosts of buffer 0 are current
-            if waf:
-                comm.wait(self._minwork)
-                sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+        if waf:
+            sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
             sw.swe_dist_flux(self.ctx, sch, 0)
-            if not waf:
-                comm.wait(self._minwork)
-                sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
-            if heun:
-                sw.swe_dist_update(self.ctx, sch, 0, 1)            # send cells of U'
-                bar1 = self._exchange_async(1)
-                sw.swe_dist_update(self.ctx, sch, 0, 2)            # the rest, behind the barrier
-                comm.wait(bar1)
-                sw.swe_dist_flux(self.ctx, sch, 1)
-                sw.swe_dist_update(self.ctx, sch, 1, 1)            # send cells of U^{n+1}
-                self._bar = self._exchange_async(0)
-                sw.swe_dist_update(self.ctx, sch, 1, 2)
-            else:
-                done = comm.allreduce_min_async(self.token) if p2p else None   # everybody's flux pass is over
-                sw.swe_dist_update(self.ctx, sch, 0, 1)
-                comm.wait(done)
-                self._bar = self._exchange_async(0)
-                sw.swe_dist_update(self.ctx, sch, 0, 2)
-            sw.swe_dist_local_min(self.ctx, self.minbuf)
-            self._minwork = comm.allreduce_min_async(self.minbuf)
+        else:                                              # rotated: flux(0) is already behind us
+            sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+        if heun:
+            sw.swe_dist_update(self.ctx, sch, 0, 1)            # send cells of U'
+            bar1 = self._exchange_async(1)
+            sw.swe_dist_update(self.ctx, sch, 0, 2)            # the rest, behind the barrier
+            comm.wait(bar1)
+            sw.swe_dist_flux(self.ctx, sch, 1)
+            sw.swe_dist_update(self.ctx, sch, 1, 1)            # send cells of U^{n+1}
+            bar = self._exchange_async(0)
+            sw.swe_dist_update(self.ctx, sch, 1, 2)
+        else:
+            done = comm.allreduce_min_async(self.token) if p2p else None   # everybody's flux pass is over
+            sw.swe_dist_update(self.ctx, sch, 0, 1)
+            comm.wait(done)
+            bar = self._exchange_async(0)
+            sw.swe_dist_update(self.ctx, sch, 0, 2)
+        sw.swe_dist_local_min(self.ctx, self.minbuf)
+        mw = comm.allreduce_min_async(self.minbuf)
+        comm.wait(bar)                                     # ghosts of buffer 0 are current
+        if not waf:
+            sw.swe_dist_flux(self.ctx, sch, 0)             # of the NEXT step, while the minimum is reduced
+        comm.wait(mw)
+
+    def step(self, nsteps, cfl, scheme):
+        """nsteps time steps, asynchronous: enqueued on the solver's stream, which is ordered
+        behind the caller's current stream; the caller's stream waits for it (no host sync)."""
+        import time as _time
+        sw = self.sw
+        sch = sw.SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
+        nsteps = int(nsteps)
+        if nsteps <= 0:
+            return
+        overlap = self.schedule == "overlap"
+        rotated = overlap and sch != sw.SWE_WAF
+        body = self._body_overlap if overlap else self._body_plain
+        t0 = _time.perf_counter()
+        with self._on_stream():
+            self._prime()
+            if rotated and self._flux_done != sch:
+                sw.swe_dist_flux(self.ctx, sch, 0)
+            self._flux_done = sch if rotated else None
+            done = 0
+            if self.graphs and nsteps >= 2 and self.tstream is not None and not self.comm.staged_host \
+                    and not self.profile:
+                key = (sch, float(cfl), self.schedule)
+                ent = self._graph.get(key)
+                if ent is None:
+                    body(sch, cfl)                         # a real step: NCCL set-up and lazy loading happen outside the capture
+                    done = 1
+                    ent = self._capture(body, sch, cfl)
+                    if ent is not None:
+                        self._graph[key] = ent
+                if ent is not None:
+                    g, dl, dh, ds = ent
+                    n = nsteps - done
+                    for _ in range(n):
+                        g.replay()
+                    sw.swe_account_replays(self.ctx, n * ds, n * dl, n * dh)
+                    self.graph_replays += n
+                    done = nsteps
+            for _ in range(nsteps - done):
+                body(sch, cfl)
+        self.host_us_per_step = 1e6 * (_time.perf_counter() - t0) / nsteps
+
+    def _capture(self, body, sch, cfl):
+        """One step captured as a CUDA graph on the solver's stream (kernels of the library and the
+        NCCL collectives alike).  Returns None -- and says so once on stderr -- if the capture
+        fails (then every step is enqueued call by call, as with gloo)."""
+        torch, sw = self.torch, self.sw
+        g = torch.cuda.CUDAGraph()
+        self.tstream.synchronize()
+        s1 = sw.swe_get_stats(self.ctx)
+        try:
+            with torch.cuda.graph(g, stream=self.tstream, capture_error_mode="thread_local"):
+                body(sch, cfl)
+        except Exception as e:                             # depends on the NCCL build
+            import sys
+            sys.stderr.write("[swe dist] rank %d: CUDA-graph capture of the step failed (%s); steps are enqueued "
+                             "call by call\n" % (self.rank, str(e).splitlines()[0] if str(e) else type(e).__name__))
+            self.graphs = False
+            g = None
+        s2 = sw.swe_get_stats(self.ctx)
+        # the captured body was recorded, not run: take its counts back out of the library's statistics
+        dl, dh, ds = (s2["kernel_launches"] - s1["kernel_launches"], s2["halo_bytes"] - s1["halo_bytes"],
+                      s2["steps"] - s1["steps"])
+        sw.swe_account_replays(self.ctx, -ds, -dl, -dh)
+        return None if g is None else (g, dl, dh, ds)
+
+    def set_profile(self, on):
+        """Per-kernel CUDA events of the library (swe_set_profile); steps are then enqueued call
+        by call (events cannot be recorded inside a replayed graph)."""
+        self.profile = bool(on)
+        with self._on_stream():
+            self.sw.swe_set_profile(self.ctx, bool(on))
 
     def _drain(self):
-        """Completes the collectives the overlap schedule left in flight (the ghosts of buffer 0 are
-        then current and minbuf holds the global minimum)."""
-        self.comm.wait(self._bar)
-        self.comm.wait(self._minwork)
-        self._bar = self._minwork = None
+        """Nothing is left in flight between steps: every collective has been waited for on the
+        stream; kept for callers of the round-1 interface."""
+        return None
 
     def time(self):
         return self.sw.swe_get_time(self.ctx)
 
     def set_state(self, h, hu, hv):
-        self._drain()
         self._primed = False
+        self._flux_done = None
         self.comm.host_barrier()
-        self.sw.swe_set_state(self.ctx, h, hu, hv)
+        with self._on_stream():
+            self.sw.swe_set_state(self.ctx, h, hu, hv)
         self.comm.host_barrier()
 
     def get_state_local(self, h, hu, hv):
         """Fills the entries of this rank's owned cells only."""
-        self.sw.swe_get_state(self.ctx, h, hu, hv)
+        with self._on_stream():
+            self.sw.swe_get_state(self.ctx, h, hu, hv)
 
     def get_state(self):
         """The full state on every rank (numpy): owned cells of all ranks summed over zero arrays."""
         torch = self.torch
         out = torch.zeros(3, self.ncell, dtype=torch.float64, device=self.minbuf.device)
-        self.sw.swe_get_state(self.ctx, out[0], out[1], out[2])
-        self.comm.allreduce_sum(out)
+        with self._on_stream():
+            self.sw.swe_get_state(self.ctx, out[0], out[1], out[2])
+            self.comm.allreduce_sum(out)
+        if self.tstream is not None:
+            self.tstream.synchronize()
         return tuple(o.cpu().numpy() for o in out)
 
     def close(self):
-        self._drain()
+        self._graph.clear()
         self.comm.host_barrier()                       # nobody still pushes into this rank's buffers
         self.sw.swe_mesh_destroy(self.ctx)
         self.ctx = None

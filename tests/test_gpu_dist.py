@@ -300,6 +300,18 @@ def _nccl_worker(port, schedule, transport, q):
         S.step(5, 0.45, "waf")
         t = S.time()
         st = S.get_state()
+        # the step ran as a replayed CUDA graph (kernels + NCCL collectives), and the library's
+        # counters saw the replays
+        stats = sw.swe_get_stats(S.ctx)
+        assert S.graph_replays == (8 - 1) + (7 - 1) + (5 - 1), S.graph_replays
+        assert stats["steps"] == 20, stats
+        S2 = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport, schedule=schedule, graphs=False)
+        S2.step(8, 0.45, "muscl"); S2.step(7, 0.9, "hllc"); S2.step(5, 0.45, "waf")
+        st_eager, t_eager = S2.get_state(), S2.time()
+        stats2 = sw.swe_get_stats(S2.ctx)
+        S2.close()
+        assert S2.graph_replays == 0 and t_eager == t and all(np.array_equal(x, y) for x, y in zip(st, st_eager))
+        assert stats2["kernel_launches"] == stats["kernel_launches"] and stats2["halo_bytes"] == stats["halo_bytes"], (stats, stats2)
         S.set_state(*[torch.from_numpy(x.copy()) for x in st])
         S.step(3, 0.45, "muscl_ms")
         st2 = S.get_state()
