@@ -256,8 +256,10 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
     from paper_2307_16758_b200 import dist as swdist
     import paper_2307_16758_b200 as sw
 
+    t_setup = time.perf_counter()
     S = swdist.DistSolver(cfg, nzones=args.zones if args.zones > 0 else None, nlayers=args.layers,
                           transport=args.transport, schedule=args.schedule, graphs=not args.no_dist_graph)
+    setup_s = swdist.reduce_max(time.perf_counter() - t_setup)     # host mesh + zones + upload + IPC, slowest rank
     nt = S.ncell
     info = sw.swe_mesh_info(S.ctx)
     owned = sum(sw.swe_zone_describe_counts(S.ctx, z)[0] for z in range(*swdist.shard_units(S.nzones, rank, world)))
@@ -329,6 +331,8 @@ def run_dist(args, rank, world, local, cfg, desc, cfl):
                                       "schedule %s, all-reduce(min) of dt" % (world, S.nzones, S.nlayers, S.transport,
                                                                               S.schedule),
                        "zones": S.nzones, "ghost_layers": S.nlayers, "halo_bytes_per_step": halo,
+                       "transport_requested": args.transport, "transport_used": S.transport,
+                       "solver_setup_s": setup_s,
                        "step_as_cuda_graph": bool(replays), "host_us_per_step": host_us,
                        "rank0_kernel_ms_per_step": kern_ms,
                        "rank0_not_in_kernels_ms_per_step": max(0.0, ms / args.steps - kern_ms),
@@ -376,6 +380,10 @@ def main():
     from paper_2307_16758_b200 import dist as swdist
     import paper_2307_16758_b200 as sw
 
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        # NCCL's communicator set-up lines (ranks, transports, NVLS) go to stderr: evidence of the N-rank run
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     rank, world, local = swdist.init_from_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
