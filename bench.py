@@ -500,6 +500,7 @@ def main():
     zstats = sw.swe_zone_stats(ctx) if args.zones > 0 else None
     if zstats:
         zstats["setup_ms"] = sw.swe_zone_setup_ms(ctx)       # row f4: device ghost layers / zone build / whole call
+        zstats["setup_detail_ms"] = sw.swe_zone_setup_detail(ctx)
     roofline["fp64_peak_TFLOPs_measured"] = sw.swe_fp64_peak(ctx)      # the other side of the roofline
     sw.swe_mesh_destroy(ctx)
 

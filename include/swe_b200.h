@@ -124,12 +124,20 @@ int swe_set_dry_masks(swe_ctx* ctx, int on);
  * The ghost layers and their numbering (sections 3.2-3.3)
  * are generated on the device: the layers of all zones grow together as bit masks over the edge
  * adjacency, one launch per layer, and a radix sort of (zone, source zone, layer, cell) keys gives
- * the contiguous receive ranges (csrc/swe_zone_kernels.cuh). */
+ * the contiguous receive ranges (csrc/swe_zone_kernels.cuh); the zones' own copies of connectivity
+ * and geometry in that numbering are then gathered on the device as well
+ * (csrc/swe_zone_assembly.cuh): the concatenated zoned mesh never exists on the host. */
 int swe_zones_create(swe_ctx* ctx, int nzones, int nlayers, const int32_t* zone_of_cell);
 /* wall-clock milliseconds of the last swe_zones_create / swe_zones_create_dist (host pointers,
- * any may be NULL): the device ghost-layer generation alone; the whole zone build up to the
- * concatenated host arrays; the whole call including the upload.  SWE_ERR_STATE without zones. */
+ * any may be NULL): the device ghost-layer generation alone; the call up to and including the
+ * host's link / exchange lists; the whole call.  SWE_ERR_STATE without zones. */
 int swe_zone_setup_ms(const swe_ctx* ctx, double* ghost_layers_ms, double* build_ms, double* total_ms);
+/* The same call broken down (host pointer, 5 doubles, milliseconds): [0] the zone of every cell
+ * (recursive coordinate bisection, or mapping the caller's array), [1] the ghost layers of all
+ * zones (device), [2] owned-cell positions (device) + links, send lists and per-rank exchange lists
+ * (host, O(ghost cells)), [3] the zones' copies of connectivity and geometry assembled on the device
+ * (swe_zone_assembly.cuh; section 3.3), [4] the whole call. */
+int swe_zone_setup_detail(const swe_ctx* ctx, double* ms);
 /* pack: send buffer[k] = U[send_idx[k]] for every link whose SOURCE is `zone` (-1 = all zones);
  * unpack: copy the buffers into the contiguous ghost ranges of `zone` (-1 = all). */
 int swe_pack_ghosts(swe_ctx* ctx, int zone);
@@ -139,7 +147,9 @@ int swe_zone_stats(const swe_ctx* ctx, int64_t* send_cells_total, int64_t* bytes
 /* description of one zone for tests and for a multi-GPU driver: counts, then the arrays.
  * cells: user ids of owned cells then ghost blocks (nowned+nghost); layer: 0 owned, l = ghost
  * layer; links (one per source zone, ascending): src zone, receive start, count; send list of a
- * link = source-zone-local indices. */
+ * link = source-zone-local indices.  swe_zone_cells serves the zones resident on this rank (the
+ * lists live on the device and are fetched the first time it is called); counts and links are
+ * known for every zone.  Errors: SWE_ERR_ARG (no zones, no such zone, zone on another rank). */
 int swe_zone_describe(const swe_ctx* ctx, int zone, int64_t* nowned, int64_t* nghost, int64_t* nlinks);
 int swe_zone_cells(const swe_ctx* ctx, int zone, int32_t* cells, int32_t* layer);
 int swe_zone_links(const swe_ctx* ctx, int zone, int32_t* src, int32_t* start, int32_t* count);

@@ -47,6 +47,7 @@ SIGNATURES = {
     "swe_unpack_ghosts": (C.c_int, [_vp, C.c_int]),
     "swe_zone_stats": (C.c_int, [_vp, _i64p, _i64p, _i64p]),
     "swe_zone_setup_ms": (C.c_int, [_vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "swe_zone_setup_detail": (C.c_int, [_vp, _dp]),
     "swe_zone_describe": (C.c_int, [_vp, C.c_int, _i64p, _i64p, _i64p]),
     "swe_zone_cells": (C.c_int, [_vp, C.c_int, _vp, _vp]),
     "swe_zone_links": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
@@ -252,6 +253,12 @@ def swe_zone_stats(ctx):
     a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
     _check(lib().swe_zone_stats(ctx, C.byref(a), C.byref(b), C.byref(c)))
     return {"send_cells_total": a.value, "bytes_per_exchange": b.value, "ghost_cells_total": c.value}
+
+
+def swe_zone_setup_detail(ctx):
+    v = (C.c_double * 5)()
+    _check(lib().swe_zone_setup_detail(ctx, v))
+    return dict(zip(["zone_of_ms", "ghost_layers_ms", "lists_ms", "assembly_ms", "total_ms"], list(v)))
 
 
 def swe_zone_setup_ms(ctx):

@@ -128,7 +128,7 @@ int64_t swe_host_get(void* hh, const char* name, void* out, int64_t cap_bytes) {
         if (n == "zone_offset" || n == "zone_nowned" || n == "zone_ncells") {
             std::vector<int64_t> v;
             for (const ZoneDesc& zd : h->Z.z)
-                v.push_back(n == "zone_offset" ? zd.offset : (n == "zone_nowned" ? zd.nowned : (int64_t)zd.cells.size()));
+                v.push_back(n == "zone_offset" ? zd.offset : (n == "zone_nowned" ? zd.nowned : zd.ncells));
             return copy_out(v, out, cap_bytes);
         }
     }

@@ -397,9 +397,16 @@ void rcb_split(const HostMesh& H, std::vector<int32_t>& ids, int z0, int nz, std
 
 }  // namespace
 
+void rcb_zones(const HostMesh& H, int nzones, std::vector<int32_t>& zone_of) {
+    std::vector<int32_t> ids(H.m.nc);
+    std::iota(ids.begin(), ids.end(), 0);
+    zone_of.assign(H.m.nc, -1);
+    rcb_split(H, ids, 0, nzones, zone_of);
+}
+
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32_t* zone_of_cell_user,
                  std::string& err, int nranks, int rank, const int32_t* zone_begin,
-                 const GhostFinder& ghost_finder) {
+                 const GhostFinder& ghost_finder, const ZoneDeviceLists* dev, bool assemble) {
     const MeshArrays& G = H.m;
     const int64_t nc = G.nc;
     Z = ZoneSet();
@@ -418,7 +425,10 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     }
     auto resident = [&](int zi) { return Z.zone_rank[zi] == rank; };
     Z.zone_of.assign(nc, -1);
-    if (zone_of_cell_user) {
+    if (dev) {
+        if ((!dev->zone_of.empty() && (int64_t)dev->zone_of.size() != nc) || (int64_t)dev->nowned.size() != nz) { err = "bad device zone lists"; return false; }
+        Z.zone_of = dev->zone_of;            // may be empty: the zone ids then live on the device only
+    } else if (zone_of_cell_user) {
         for (int64_t i = 0; i < nc; ++i) {
             int32_t zc = zone_of_cell_user[G.cell_user[i]];
             if (zc < 0 || zc >= nz) { err = "zone_of_cell value out of range"; return false; }
@@ -426,16 +436,19 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         }
     } else {
         if (nz & (nz - 1)) { err = "recursive coordinate bisection needs a power-of-two nzones"; return false; }
-        std::vector<int32_t> ids(nc);
-        std::iota(ids.begin(), ids.end(), 0);
-        rcb_split(H, ids, 0, nz, Z.zone_of);
+        rcb_zones(H, nz, Z.zone_of);
     }
     Z.z.assign(nz, ZoneDesc());
-    std::vector<int32_t> owned_pos(nc);
-    for (int64_t i = 0; i < nc; ++i) {          // owned cells in ascending device id
-        ZoneDesc& zd = Z.z[Z.zone_of[i]];
-        owned_pos[i] = (int32_t)zd.cells.size();
-        zd.cells.push_back((int32_t)i);
+    std::vector<int32_t> owned_pos(dev ? 0 : nc);
+    if (dev) {
+        for (int zi = 0; zi < nz; ++zi) Z.z[zi].nowned = dev->nowned[zi];
+    } else {
+        for (int64_t i = 0; i < nc; ++i) {      // owned cells in ascending device id
+            ZoneDesc& zd = Z.z[Z.zone_of[i]];
+            owned_pos[i] = (int32_t)zd.cells.size();
+            zd.cells.push_back((int32_t)i);
+        }
+        for (int zi = 0; zi < nz; ++zi) Z.z[zi].nowned = (int64_t)Z.z[zi].cells.size();
     }
     // A.12.2 ghost layers = breadth-first distance over the edge adjacency; A.12.3 numbering.
     // From the device generator (sorted keys of all zones) when the library runs, by the host
@@ -445,19 +458,22 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         if ((int64_t)nz * nz > (int64_t)1 << 29) { err = "too many zones"; return false; }
         if (!ghost_finder(Z.zone_of, nz, nlayers, keys, err)) return false;
     }
+    if (dev && (!ghost_finder || dev->key_owned_pos.size() != keys.size())) { err = "bad device zone lists (keys)"; return false; }
     size_t kpos = 0;
     std::vector<int32_t> mark(ghost_finder ? 0 : nc, -1);
-    struct Gh { int32_t cell, layer, src; };
+    struct Gh { int32_t cell, layer, src, opos; };
     for (int zi = 0; zi < nz; ++zi) {
         ZoneDesc& zd = Z.z[zi];
-        zd.nowned = (int64_t)zd.cells.size();
         zd.layer.assign(zd.cells.size(), 0);
+        int64_t cur = zd.nowned;                 // next local index
         std::vector<Gh> ghosts;
         if (ghost_finder) {
             for (; kpos < keys.size(); ++kpos) {
                 const uint64_t b = keys[kpos] >> 32;
                 if ((int64_t)((b >> 2) / (uint64_t)nz) != zi) break;
-                ghosts.push_back(Gh{(int32_t)(keys[kpos] & 0xffffffffu), (int32_t)(b & 3), (int32_t)((b >> 2) % (uint64_t)nz)});
+                const int32_t cell = (int32_t)(keys[kpos] & 0xffffffffu);
+                ghosts.push_back(Gh{cell, (int32_t)(b & 3), (int32_t)((b >> 2) % (uint64_t)nz),
+                                    dev ? dev->key_owned_pos[kpos] : owned_pos[cell]});
             }
         } else {
             for (int32_t i : zd.cells) mark[i] = zi;
@@ -469,7 +485,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
                         int32_t nbq = G.c2c[4 * (int64_t)i + k];
                         if (nbq >= 0 && mark[nbq] != zi) {
                             mark[nbq] = zi; next.push_back(nbq);
-                            ghosts.push_back(Gh{nbq, l, Z.zone_of[nbq]});
+                            ghosts.push_back(Gh{nbq, l, Z.zone_of[nbq], owned_pos[nbq]});
                         }
                     }
                 frontier.swap(next);
@@ -481,22 +497,23 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         }
         for (const Gh& gq : ghosts) {
             if (zd.links.empty() || zd.links.back().src != gq.src) {
-                ZoneLink lk; lk.src = gq.src; lk.start = (int32_t)zd.cells.size(); lk.count = 0;
+                ZoneLink lk; lk.src = gq.src; lk.start = (int32_t)cur; lk.count = 0;
                 zd.links.push_back(lk);
             }
             ZoneLink& lk = zd.links.back();
             lk.count++;
-            lk.send.push_back(owned_pos[gq.cell]);
-            zd.cells.push_back(gq.cell);
-            zd.layer.push_back(gq.layer);
+            lk.send.push_back(gq.opos);
+            if (!dev) { zd.cells.push_back(gq.cell); zd.layer.push_back(gq.layer); }
+            ++cur;
         }
+        zd.ncells = cur;
     }
     if (kpos != keys.size()) { err = "ghost keys are not sorted by zone"; return false; }
     // offset of every zone in the concatenated mesh of the rank that holds it
     std::vector<int64_t> owner_off(nz, 0), rank_cells(nranks, 0);
     for (int zi = 0; zi < nz; ++zi) {
         owner_off[zi] = rank_cells[Z.zone_rank[zi]];
-        rank_cells[Z.zone_rank[zi]] += (int64_t)Z.z[zi].cells.size();
+        rank_cells[Z.zone_rank[zi]] += Z.z[zi].ncells;
         Z.z[zi].offset = resident(zi) ? owner_off[zi] : -1;
     }
     const int64_t ncz = rank_cells[rank];
@@ -504,9 +521,10 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         if (rank_cells[r] > (int64_t)INT32_MAX / 4) { err = "zoned mesh too large"; return false; }
     if (ncz > (int64_t)INT32_MAX / 4) { err = "zoned mesh too large"; return false; }
 
+    MeshArrays& M = Z.mesh;
+    if (assemble) {
     // ---- concatenated zoned mesh ----
     const int gl = (nlayers >= 2) ? 1 : 0;   // gradients are needed on layers <= gl (A.12.5)
-    MeshArrays& M = Z.mesh;
     M.nc = ncz;
     M.cell_user.resize(ncz); M.c2c.assign(4 * ncz, 0); M.c2e.assign(4 * ncz, 0);
     M.zc.resize(ncz); M.area.resize(ncz); M.rin.resize(ncz);
@@ -598,6 +616,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         }
         for (size_t j = 0; j < zd.cells.size(); ++j) loc[zd.cells[j]] = -1;
     }
+    }   // assemble
     // ---- flattened exchange lists: links between two resident zones ----
     Z.link_off.push_back(0);
     for (int zi = 0; zi < nz; ++zi) {
@@ -641,7 +660,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
         Z.send_cells.insert(Z.send_cells.end(), Z.send_idx.begin(), Z.send_idx.end());
         std::sort(Z.send_cells.begin(), Z.send_cells.end());
         Z.send_cells.erase(std::unique(Z.send_cells.begin(), Z.send_cells.end()), Z.send_cells.end());
-        for (int32_t c : Z.send_cells) M.c2e[4 * (int64_t)c + 3] = -1;
+        if (assemble) for (int32_t c : Z.send_cells) M.c2e[4 * (int64_t)c + 3] = -1;
     }
     return true;
 }

@@ -43,6 +43,7 @@ struct ZoneLink {
 };
 struct ZoneDesc {
     int64_t nowned = 0;
+    int64_t ncells = 0;                      // owned + ghost cells
     int64_t offset = 0;                      // first cell of the zone in the concatenated mesh
     std::vector<int32_t> cells;              // global DEVICE ids (un-zoned mesh): owned, then ghosts
     std::vector<int32_t> layer;
@@ -97,8 +98,22 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
 // search below (the host-inspection entry points, which must run without a GPU).
 using GhostFinder = std::function<bool(const std::vector<int32_t>& zone_of, int nzones, int nlayers,
                                        std::vector<uint64_t>& keys, std::string& err)>;
+// The library's device path (row f4, swe_zone_assembly.cuh) takes over what is O(cells) here: it
+// hands in the zone of every cell, the number of owned cells per zone and, per ghost key, the
+// position of that cell among its owner's cells (`ZoneDeviceLists`), gets the links and exchange
+// lists back, and assembles the concatenated zoned mesh on the device itself (assemble = false:
+// ZoneSet::mesh, src_of_cell and the owned part of ZoneDesc::cells / layer are then left empty;
+// ZoneDesc::ncells always holds the count).
+struct ZoneDeviceLists {
+    std::vector<int32_t> zone_of;            // per cell of the un-zoned mesh, device numbering (may be left empty)
+    std::vector<int64_t> nowned;             // per zone
+    std::vector<int32_t> key_owned_pos;      // per ghost key: index of the cell among its owner zone's cells
+};
 bool build_zones(const HostMesh& H, ZoneSet& Z, int nzones, int nlayers,
                  const int32_t* zone_of_cell_user, std::string& err, int nranks = 1, int rank = 0,
-                 const int32_t* zone_begin = nullptr, const GhostFinder& ghost_finder = GhostFinder());
+                 const int32_t* zone_begin = nullptr, const GhostFinder& ghost_finder = GhostFinder(),
+                 const ZoneDeviceLists* dev = nullptr, bool assemble = true);
+// RCB of A.12.1 on the host (used by build_zones when no zone_of_cell is given and by the tests)
+void rcb_zones(const HostMesh& H, int nzones, std::vector<int32_t>& zone_of);
 
 }  // namespace swe

@@ -4,6 +4,7 @@
 #include "host_mesh.hpp"
 #include "swe_kernels.cuh"
 #include "swe_zone_kernels.cuh"
+#include "swe_zone_assembly.cuh"
 
 #include <chrono>
 #include <cmath>
@@ -66,6 +67,18 @@ struct Store {
     }
 };
 
+// device temporaries of a set-up call, freed on every way out
+struct Scratch {
+    std::vector<void*> p;
+    template <class T> cudaError_t get(T** q, size_t n) {
+        void* v = nullptr;
+        cudaError_t e = cudaMalloc(&v, (n ? n : 1) * sizeof(T));
+        if (e == cudaSuccess) { p.push_back(v); *q = (T*)v; }
+        return e;
+    }
+    ~Scratch() { for (void* v : p) cudaFree(v); }
+};
+
 }  // namespace
 
 struct swe_ctx {
@@ -97,7 +110,10 @@ struct swe_ctx {
     double4** d_peerB = nullptr;
     std::vector<void*> peerA, peerB;   // host copies; [rank] = this context's own buffers
     std::vector<char> peer_ipc;        // 1: opened with cudaIpcOpenMemHandle (closed in free_zones)
-    double zone_ms[3] = {0, 0, 0};     // last swe_zones_create: device ghost layers, + host zone build, + upload (cumulative)
+    std::vector<int> zr_zone;          // resident zones and their first cell in the concatenated mesh
+    std::vector<long long> zr_off;     // (the zones' cell lists are downloaded on demand)
+    bool zone_cells_on_host = false;
+    double zone_ms[5] = {0, 0, 0, 0, 0};     // last swe_zones_create: device ghost layers, + host zone build, + upload (cumulative)
     int* d_send_cells = nullptr;       // distinct cells on a send list (overlap schedule updates them first)
     int64_t nsendcells = 0;
     // staging for host pointers
@@ -312,6 +328,8 @@ void free_zones(swe_ctx* c) {
     c->d_sendbuf = nullptr;
     c->nsend = 0;
     c->has_zones = false;
+    c->zone_cells_on_host = false;
+    c->zr_zone.clear(); c->zr_off.clear();
     c->Z = ZoneSet();
 }
 
@@ -1012,28 +1030,29 @@ int swe_account_replays(swe_ctx* c, int64_t steps, int64_t kernel_launches, int6
 // ---- zones ----
 // Row f4: the ghost layers of all zones on the device (swe_zone_kernels.cuh).  zone_of: per cell of
 // the un-zoned mesh, device numbering.  Returns the sorted keys build_zones consumes.
-static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, int nz, int nlayers,
-                              std::vector<uint64_t>& keys, std::string& err) {
+// d_zone: the zone of every cell, already on the device.  keep != nullptr: the sorted keys also stay
+// on the device (*keep = their allocation, *d_sorted = the keys; the caller frees *keep).
+static bool device_ghost_keys(swe_ctx* c, const int* d_zone, int nz, int nlayers, std::vector<uint64_t>& keys,
+                              std::string& err, void** keep = nullptr, unsigned long long** d_sorted = nullptr) {
     const int nc = (int)c->g.nc;
     const int W = (nz + 63) / 64;
     const size_t words = (size_t)W * nc;
-    // one arena for the masks (two reach buffers, one fresh buffer per layer), the two counters and
-    // the zone ids; a second one, sized once the number of ghosts is known, for the keys
+    // one arena for the masks (two reach buffers, one fresh buffer per layer) and the two counters;
+    // a second one, sized once the number of ghosts is known, for the keys
     unsigned long long *arena = nullptr, *karena = nullptr;
     cudaError_t e = cudaSuccess;
     auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
     keys.clear();
+    if (keep) { *keep = nullptr; *d_sorted = nullptr; }
     const int grid = grid_for(nc, c->grid_light);
     unsigned long long total = 0;
     const size_t nmask = (size_t)(2 + nlayers) * words;
-    ok(cudaMalloc((void**)&arena, (nmask + 2) * 8 + (size_t)nc * sizeof(int)));
+    ok(cudaMalloc((void**)&arena, (nmask + 2) * 8));
     unsigned long long* d_reach[2] = {arena, arena + words};
     unsigned long long* d_fresh[3] = {nullptr, nullptr, nullptr};
     for (int l = 0; l < nlayers; ++l) d_fresh[l] = arena + (size_t)(2 + l) * words;
     unsigned long long* d_count = arena + nmask;             // [0] ghosts found, [1] emit cursor
-    int* d_zone = (int*)(arena + nmask + 2);
     if (e == cudaSuccess) {
-        ok(cudaMemcpyAsync(d_zone, zone_of.data(), (size_t)nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         ok(cudaMemsetAsync(d_count, 0, 2 * sizeof(unsigned long long), c->stream));
         k_gl_seed<<<grid, 256, 0, c->stream>>>(d_zone, d_reach[0], nc, W);
         for (int l = 0; l < nlayers; ++l)
@@ -1059,7 +1078,7 @@ static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, i
             for (int shift = 0; shift < bits; shift += 8) {
                 k_rs_hist<<<nblk, RS_THREADS, 0, c->stream>>>(d_keys[cur], n, shift, d_hist, nblk);
                 k_rs_scan<<<1, 1024, 0, c->stream>>>(d_hist, (long long)256 * nblk);
-                k_rs_scatter<<<nblk, RS_THREADS, 0, c->stream>>>(d_keys[cur], d_keys[cur ^ 1], n, shift, d_hist, nblk);
+                k_rs_scatter<false><<<nblk, RS_THREADS, 0, c->stream>>>(d_keys[cur], d_keys[cur ^ 1], n, shift, d_hist, nblk);
                 cur ^= 1;
                 c->launches += 3;
             }
@@ -1068,11 +1087,80 @@ static bool device_ghost_keys(swe_ctx* c, const std::vector<int32_t>& zone_of, i
             keys.resize((size_t)n);
             ok(cudaMemcpyAsync(keys.data(), d_keys[cur], (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream));
             ok(cudaStreamSynchronize(c->stream));
+            if (keep && e == cudaSuccess) { *keep = karena; *d_sorted = d_keys[cur]; karena = nullptr; }
         }
     }
     cudaFree(arena); cudaFree(karena);
     if (e != cudaSuccess) { cudaGetLastError(); err = std::string("device ghost-layer generation: ") + cudaGetErrorString(e); return false; }
     return true;
+}
+
+// stable LSD radix sort of n 64-bit keys on bits [lo_bit, hi_bit): returns 0 / 1 = the buffer that holds the result
+static int rs_sort(swe_ctx* c, unsigned long long* buf[2], long long n, int lo_bit, int hi_bit, unsigned int* d_hist,
+                   unsigned int* val[2] = nullptr) {
+    const int nblk = (int)((n + RS_TILE - 1) / RS_TILE);
+    int cur = 0;
+    for (int shift = lo_bit; shift < hi_bit; shift += 8) {
+        k_rs_hist<<<nblk, RS_THREADS, 0, c->stream>>>(buf[cur], n, shift, d_hist, nblk);
+        k_rs_scan<<<1, 1024, 0, c->stream>>>(d_hist, (long long)256 * nblk);
+        if (val) k_rs_scatter<true><<<nblk, RS_THREADS, 0, c->stream>>>(buf[cur], buf[cur ^ 1], n, shift, d_hist, nblk, val[cur], val[cur ^ 1]);
+        else k_rs_scatter<false><<<nblk, RS_THREADS, 0, c->stream>>>(buf[cur], buf[cur ^ 1], n, shift, d_hist, nblk);
+        cur ^= 1;
+        c->launches += 3;
+    }
+    return cur;
+}
+static int bits_of(unsigned long long v) { int b = 0; for (; v; v >>= 1) ++b; return b; }
+
+// A.12.1 on the device (swe_zone_assembly.cuh): d_zone[cell] = zone of every cell, nz a power of two
+static int device_rcb(swe_ctx* c, int nz, int* d_zone) {
+    const int nc = (int)c->g.nc;
+    const int grid = grid_for(nc, c->grid_light);
+    if (nz == 1) { CU(cudaMemsetAsync(d_zone, 0, (size_t)nc * sizeof(int), c->stream)); return SWE_OK; }
+    Scratch tmp;
+    unsigned long long* k[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};     // [axis][ping-pong]
+    unsigned int* v[2] = {nullptr, nullptr};
+    unsigned int* d_hist = nullptr;
+    int* d_user_cell = nullptr;
+    long long* d_seg = nullptr;
+    double* d_c[2] = {nullptr, nullptr};
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) CU(tmp.get(&k[a][b], (size_t)nc));
+    CU(tmp.get(&v[0], (size_t)nc)); CU(tmp.get(&v[1], (size_t)nc));
+    CU(tmp.get(&d_hist, (size_t)256 * (size_t)((nc + RS_TILE - 1) / RS_TILE)));
+    CU(tmp.get(&d_user_cell, (size_t)nc)); CU(tmp.get(&d_seg, (size_t)nz + 1)); CU(tmp.get(&d_c[0], (size_t)nc)); CU(tmp.get(&d_c[1], (size_t)nc));
+    CU(cudaMemcpyAsync(d_user_cell, c->H.user_cell.data(), (size_t)nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(d_c[0], c->H.cx.data(), (size_t)nc * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(d_c[1], c->H.cy.data(), (size_t)nc * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    int cur[2] = {0, 0};
+    for (int a = 0; a < 2; ++a) {                    // the two global orders
+        k_rcb_init<<<grid, 256, 0, c->stream>>>(d_user_cell, d_c[a], k[a][0], v[0], nc);
+        const int r = rs_sort(c, k[a], nc, 0, 64, d_hist, v);
+        k_rcb_order<<<grid, 256, 0, c->stream>>>(v[r], k[a][0], nc);
+        cur[a] = 0;
+    }
+    std::vector<long long> seg{0, nc};
+    int levels = 0;
+    for (int m = nz; m > 1; m >>= 1) ++levels;
+    for (int l = 0; l < levels; ++l) {
+        const int nseg = (int)seg.size() - 1;
+        CU(cudaMemcpyAsync(d_seg, seg.data(), seg.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+        k_rcb_mark<<<grid, 256, 0, c->stream>>>(k[0][cur[0]], k[1][cur[1]], d_c[0], d_c[1], d_seg, nseg, d_zone, nc);
+        for (int a = 0; a < 2; ++a) {
+            k_rcb_rekey<<<grid, 256, 0, c->stream>>>(k[a][cur[a]], d_zone, nc);
+            unsigned long long* pp[2] = {k[a][cur[a]], k[a][cur[a] ^ 1]};
+            const int r = rs_sort(c, pp, nc, 32, 32 + l + 1, d_hist);
+            cur[a] ^= r;
+        }
+        CU(cudaStreamSynchronize(c->stream));          // seg is re-uploaded next level
+        std::vector<long long> nxt;
+        for (int s2 = 0; s2 < nseg; ++s2) { nxt.push_back(seg[s2]); nxt.push_back(seg[s2] + (seg[s2 + 1] - seg[s2]) / 2); }
+        nxt.push_back(nc);
+        seg.swap(nxt);
+        c->launches += 3;
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
 }
 
 static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t* zone_of_cell, int nranks,
@@ -1094,39 +1182,246 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     std::string err;
     bool ok = false;
     const auto t0 = std::chrono::steady_clock::now();
-    double ghost_ms = 0.0;
-    GhostFinder finder = [&](const std::vector<int32_t>& zone_of, int nz, int nl, std::vector<uint64_t>& keys, std::string& er) {
-        const auto g0 = std::chrono::steady_clock::now();
-        const bool r = device_ghost_keys(c, zone_of, nz, nl, keys, er);
-        ghost_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - g0).count();
-        return r;
+    auto ms_since = [&](std::chrono::steady_clock::time_point a) {
+        return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - a).count(); };
+    Scratch tmp;
+    const bool trace = getenv("SWE_ZONE_TRACE") != nullptr;
+    auto mark = [&](const char* what) {
+        if (!trace) return;
+        cudaStreamSynchronize(c->stream);
+        fprintf(stderr, "[swe zones] %-28s %8.1f ms\n", what, ms_since(t0));
     };
-    try { ok = build_zones(c->H, c->Z, nzones, nlayers, zone_of_cell, err, nranks, rank, zone_begin, finder); }
+    const int nc = (int)c->g.nc;
+    const int nz = nzones;
+    if (nlayers < 1 || nlayers > 3) return fail(SWE_ERR_ARG, "nlayers must be 1, 2 or 3");
+    if ((int64_t)nz * nz > (int64_t)1 << 29) return fail(SWE_ERR_ARG, "too many zones");
+    const int grid = grid_for(nc, c->grid_light);
+
+    // ---- A.12.1 the zone of every cell (device numbering) ----
+    ZoneDeviceLists dev;
+    if (zone_of_cell) {
+        dev.zone_of.resize(nc);
+        for (int i = 0; i < nc; ++i) {
+            const int32_t zc = zone_of_cell[c->H.m.cell_user[i]];
+            if (zc < 0 || zc >= nz) return fail(SWE_ERR_ARG, "zone_of_cell value out of range");
+            dev.zone_of[i] = zc;
+        }
+    }
+    int* d_zone = nullptr;
+    CU(tmp.get(&d_zone, (size_t)nc));
+    if (zone_of_cell) {
+        CU(cudaMemcpyAsync(d_zone, dev.zone_of.data(), (size_t)nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    } else {
+        if (nz & (nz - 1)) return fail(SWE_ERR_ARG, "recursive coordinate bisection needs a power-of-two nzones");
+        rc = device_rcb(c, nz, d_zone); if (rc) return rc;       // the zone ids stay on the device
+    }
+    c->zone_ms[3] = ms_since(t0);
+
+    mark("zone of every cell");
+    // ---- A.12.2-3 ghost layers of all zones: sorted keys, on the host and still on the device ----
+    std::vector<uint64_t> hkeys;
+    void* keep = nullptr; unsigned long long* d_gkeys = nullptr;
+    const auto g0 = std::chrono::steady_clock::now();
+    if (!device_ghost_keys(c, d_zone, nz, nlayers, hkeys, err, &keep, &d_gkeys)) return fail(SWE_ERR_CUDA, err);
+    if (keep) tmp.p.push_back(keep);
+    c->zone_ms[0] = ms_since(g0);
+    const long long nk = (long long)hkeys.size();
+
+    mark("ghost layers");
+    // ---- owned cells: one stable radix pass per 8 zone bits over (zone << 32 | cell) ----
+    unsigned long long* okeys[2] = {nullptr, nullptr};
+    unsigned int* d_hist = nullptr;
+    long long* d_start = nullptr;
+    int *d_opos = nullptr, *d_kopos = nullptr;
+    CU(tmp.get(&okeys[0], (size_t)nc)); CU(tmp.get(&okeys[1], (size_t)nc));
+    CU(tmp.get(&d_start, (size_t)nz + 1));
+    CU(tmp.get(&d_opos, (size_t)nc));
+    CU(tmp.get(&d_kopos, (size_t)nk));
+    const long long ne_int_g = c->g.dm.ne_int;
+    {
+        const long long nmax = std::max<long long>(std::max<long long>(nc, 2 * ne_int_g), 1);
+        CU(tmp.get(&d_hist, (size_t)256 * (size_t)((nmax + RS_TILE - 1) / RS_TILE)));
+    }
+    k_za_owned_keys<<<grid, 256, 0, c->stream>>>(d_zone, okeys[0], nc);
+    const int ocur = rs_sort(c, okeys, nc, 32, 32 + bits_of((unsigned long long)nz - 1), d_hist);
+    CU(cudaMemsetAsync(d_start, 0xff, ((size_t)nz + 1) * sizeof(long long), c->stream));
+    k_za_starts<<<grid, 256, 0, c->stream>>>(okeys[ocur], nc, d_start);
+    std::vector<long long> ostart((size_t)nz + 1);
+    CU(cudaMemcpyAsync(ostart.data(), d_start, ((size_t)nz + 1) * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    ostart[nz] = nc;
+    for (int z = nz - 1; z >= 0; --z) if (ostart[z] < 0) ostart[z] = ostart[z + 1];       // zones without cells
+    CU(cudaMemcpyAsync(d_start, ostart.data(), ((size_t)nz + 1) * sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+    k_za_owned_pos<<<grid, 256, 0, c->stream>>>(okeys[ocur], d_start, d_opos, nc);
+    dev.nowned.resize(nz);
+    for (int z = 0; z < nz; ++z) dev.nowned[z] = ostart[z + 1] - ostart[z];
+    dev.key_owned_pos.resize((size_t)nk);
+    if (nk) {
+        k_za_key_opos<<<grid_for(nk, c->grid_light), 256, 0, c->stream>>>(d_gkeys, nk, d_opos, d_kopos);
+        CU(cudaMemcpyAsync(dev.key_owned_pos.data(), d_kopos, (size_t)nk * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(c->stream));
+    c->launches += 4;
+
+    mark("owned positions");
+    // ---- links, send lists, exchange lists per rank: the host, from the keys (O(ghost cells)) ----
+    GhostFinder finder = [&](const std::vector<int32_t>&, int, int, std::vector<uint64_t>& keys, std::string&) {
+        keys = hkeys; return true; };
+    try { ok = build_zones(c->H, c->Z, nz, nlayers, nullptr, err, nranks, rank, zone_begin, finder, &dev, false); }
     catch (const std::bad_alloc&) { c->Z = ZoneSet(); return fail(SWE_ERR_NOMEM, "out of host memory in zone set-up"); }
     if (!ok) { c->Z = ZoneSet(); return fail(SWE_ERR_ARG, err); }
-    c->zone_ms[0] = ghost_ms;
-    c->zone_ms[1] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
-    rc = upload_store(c, c->z, c->Z.mesh);
-    if (rc) { free_zones(c); return rc; }
-    c->z.dm.glayer = (nlayers >= 2) ? 1 : 0;
-    {   // ghost layer per cell as bytes
-        std::vector<uint8_t> lay((size_t)c->z.nc);
-        for (int64_t i = 0; i < c->z.nc; ++i) lay[i] = (uint8_t)c->Z.mesh.c2c[4 * i + 3];
-        uint8_t* d_lay;
-        CU(c->z.upload(&d_lay, lay.data(), lay.size(), c->stream));
-        c->z.dm.layer = d_lay;
+    c->zone_ms[1] = ms_since(t0);
+
+    mark("host lists");
+    // ---- the concatenated zoned mesh, assembled on the device (swe_zone_assembly.cuh) ----
+    std::vector<int> zres(nz, -1), zid;
+    std::vector<long long> coff, nown, ownstart, ghstart, ghend;
+    {
+        size_t kp = 0;
+        for (int z = 0; z < nz; ++z) {
+            const size_t k0 = kp;
+            while (kp < hkeys.size() && (int64_t)(((hkeys[kp] >> 32) >> 2) / (uint64_t)nz) == z) ++kp;
+            if (c->Z.zone_rank[z] != rank) continue;
+            zres[z] = (int)zid.size(); zid.push_back(z);
+            coff.push_back(c->Z.z[z].offset); nown.push_back(c->Z.z[z].nowned); ownstart.push_back(ostart[z]);
+            ghstart.push_back((long long)k0); ghend.push_back((long long)kp);
+        }
     }
+    const int nzr = (int)zid.size();
+    long long ncz = 0;
+    for (int r = 0; r < nzr; ++r) ncz = std::max(ncz, coff[r] + c->Z.z[zid[r]].ncells);
+    coff.push_back(ncz);
+    if (nzr == 0 || ncz == 0) return fail(SWE_ERR_ARG, "this rank holds no zone");
+    ZoneTabs T{};
+    T.nz = nz; T.nzr = nzr; T.nlayers = nlayers; T.gl = (nlayers >= 2) ? 1 : 0;
+    int *d_zres = nullptr, *d_zid = nullptr;
+    long long* d_tab = nullptr;                      // coff | nown | ownstart | ghstart | ghend | ioff | boff
+    const size_t TS = (size_t)nzr + 1;
+    CU(tmp.get(&d_zres, (size_t)nz)); CU(tmp.get(&d_zid, (size_t)nzr)); CU(tmp.get(&d_tab, 7 * TS));
+    CU(cudaMemcpyAsync(d_zres, zres.data(), (size_t)nz * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(d_zid, zid.data(), (size_t)nzr * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    auto put_tab = [&](int slot, const std::vector<long long>& v) {
+        return cudaMemcpyAsync(d_tab + slot * TS, v.data(), v.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream); };
+    CU(put_tab(0, coff)); CU(put_tab(1, nown)); CU(put_tab(2, ownstart)); CU(put_tab(3, ghstart)); CU(put_tab(4, ghend));
+    T.zres = d_zres; T.zid = d_zid; T.coff = d_tab; T.nown = d_tab + TS; T.ownstart = d_tab + 2 * TS;
+    T.ghstart = d_tab + 3 * TS; T.ghend = d_tab + 4 * TS; T.ioff = d_tab + 5 * TS; T.boff = d_tab + 6 * TS;
+
+    Store& st = c->z;
+    st.nc = ncz;
+    int* d_src = nullptr; uint8_t* d_lay = nullptr;
+    CU(cudaMalloc((void**)&c->d_src_of_cell, (size_t)ncz * sizeof(int)));
+    d_src = c->d_src_of_cell;
+    CU(st.alloc(&d_lay, (size_t)ncz));
+    const int gridz = grid_for(ncz, c->grid_light);
+    k_za_cells<<<gridz, 256, 0, c->stream>>>(T, okeys[ocur], d_gkeys, d_src, d_lay, (int)ncz);
+
+    mark("cells");
+    // edges: count, emit, sort by (zone, global edge)
+    unsigned long long* d_cnt = nullptr;
+    CU(tmp.get(&d_cnt, 4));
+    CU(cudaMemsetAsync(d_cnt, 0, 4 * sizeof(unsigned long long), c->stream));
+    k_za_int_edges<<<grid_for(ne_int_g, c->grid_light), 256, 0, c->stream>>>(T, d_zone, c->g.dm.elr, (int)ne_int_g, nullptr, d_cnt);
+    k_za_bnd_edges<<<gridz, 256, 0, c->stream>>>(T, d_src, d_lay, c->g.dm.c2c, (int)ncz, nullptr, d_cnt + 1);
+    unsigned long long cnt[2] = {0, 0};
+    CU(cudaMemcpyAsync(cnt, d_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const long long ni = (long long)cnt[0], nb = (long long)cnt[1];
+    if (ni + nb > (long long)INT32_MAX / 2) return fail(SWE_ERR_ARG, "zoned mesh too large");
+    unsigned long long *ikeys[2] = {nullptr, nullptr}, *bkeys[2] = {nullptr, nullptr};
+    CU(tmp.get(&ikeys[0], (size_t)ni)); CU(tmp.get(&ikeys[1], (size_t)ni));
+    CU(tmp.get(&bkeys[0], (size_t)nb)); CU(tmp.get(&bkeys[1], (size_t)nb));
+    k_za_int_edges<<<grid_for(ne_int_g, c->grid_light), 256, 0, c->stream>>>(T, d_zone, c->g.dm.elr, (int)ne_int_g, ikeys[0], d_cnt + 2);
+    k_za_bnd_edges<<<gridz, 256, 0, c->stream>>>(T, d_src, d_lay, c->g.dm.c2c, (int)ncz, bkeys[0], d_cnt + 3);
+    const int kbits = 32 + bits_of((unsigned long long)nzr - 1);
+    const int icur = ni ? rs_sort(c, ikeys, ni, 0, kbits, d_hist) : 0;
+    const int bcur = nb ? rs_sort(c, bkeys, nb, 0, kbits, d_hist) : 0;
+    mark("edge keys sorted");
+    // per-zone ranges of the two sorted edge lists
+    std::vector<long long> ioff(TS), boff(TS);
+    {
+        long long* d_es = nullptr;
+        CU(tmp.get(&d_es, 2 * TS));
+        CU(cudaMemsetAsync(d_es, 0xff, 2 * TS * sizeof(long long), c->stream));
+        if (ni) k_za_starts<<<grid_for(ni, c->grid_light), 256, 0, c->stream>>>(ikeys[icur], ni, d_es);
+        if (nb) k_za_starts<<<grid_for(nb, c->grid_light), 256, 0, c->stream>>>(bkeys[bcur], nb, d_es + TS);
+        CU(cudaMemcpyAsync(ioff.data(), d_es, TS * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(boff.data(), d_es + TS, TS * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        ioff[nzr] = ni; boff[nzr] = nb;
+        for (int r = nzr - 1; r >= 0; --r) { if (ioff[r] < 0) ioff[r] = ioff[r + 1]; if (boff[r] < 0) boff[r] = boff[r + 1]; }
+        for (size_t r = 0; r < TS; ++r) boff[r] += ni;                  // boundary edges follow all interior edges
+        CU(put_tab(5, ioff)); CU(put_tab(6, boff));
+    }
+    const long long nez = ni + nb;
+    st.ne = nez; st.nbe = nb;
+    DevMesh& d = st.dm;
+    d = DevMesh{};
+    d.nc = (int)ncz; d.ne = (int)nez; d.ne_int = (int)ni; d.glayer = T.gl;
+    ZoneCellOut CO{}; ZoneEdgeOut EO{};
+    CU(st.alloc(&CO.c2c, (size_t)ncz)); CU(st.alloc(&CO.c2e, (size_t)ncz)); CU(st.alloc(&CO.cell_user, (size_t)ncz));
+    CU(st.alloc(&CO.zc, (size_t)ncz)); CU(st.alloc(&CO.area, (size_t)ncz)); CU(st.alloc(&CO.rin, (size_t)ncz));
+    CU(st.alloc(&CO.dupw, (size_t)ncz));
+    for (int k = 0; k < 3; ++k) { CU(st.alloc(&CO.w[k], (size_t)ncz)); CU(st.alloc(&CO.r[k], (size_t)ncz)); }
+    CU(st.alloc(&EO.elr, (size_t)nez)); CU(st.alloc(&EO.en, (size_t)nez)); CU(st.alloc(&EO.elen, (size_t)nez));
+    CU(st.alloc(&EO.edx, (size_t)nez)); CU(st.alloc(&EO.erl, (size_t)nez)); CU(st.alloc(&EO.err, (size_t)nez));
+    CU(st.alloc(&EO.edlr, (size_t)nez)); CU(st.alloc(&EO.ernorm, (size_t)nez)); CU(st.alloc(&EO.eside, (size_t)nez));
+    int* d_gedge = nullptr;
+    CU(tmp.get(&d_gedge, (size_t)nb));
+    EO.gedge = d_gedge;
+    k_za_fill_cells<<<gridz, 256, 0, c->stream>>>(T, c->g.dm, c->g.d_cell_user, d_zone, d_opos, d_gkeys, ikeys[icur], bkeys[bcur],
+                                                  d_src, d_lay, CO, (int)ncz, ni);
+    k_za_fill_edges<<<grid_for(nez, c->grid_light), 256, 0, c->stream>>>(T, c->g.dm, d_zone, d_opos, d_gkeys, ikeys[icur], bkeys[bcur],
+                                                                         EO, ni, nez);
+    c->launches += 7;
+    CU(cudaGetLastError());
+    d.c2c = CO.c2c; d.c2e = CO.c2e; d.zc = CO.zc; d.area = CO.area; d.rin = CO.rin; d.dupw = CO.dupw;
+    for (int k = 0; k < 3; ++k) { d.w[k] = CO.w[k]; d.r[k] = CO.r[k]; }
+    d.elr = EO.elr; d.en = EO.en; d.elen = EO.elen; d.edx = EO.edx; d.erl = EO.erl; d.err = EO.err;
+    d.edlr = EO.edlr; d.ernorm = EO.ernorm; d.eside = EO.eside;
+    d.layer = d_lay;
+    st.d_cell_user = CO.cell_user;
+    mark("arrays filled");
+    // cells on a send list carry -1 in c2e.w (overlap schedule)
+    c->nsendcells = (int64_t)c->Z.send_cells.size();
+    CU(cudaMalloc((void**)&c->d_send_cells, (size_t)(c->nsendcells ? c->nsendcells : 1) * sizeof(int)));
+    if (c->nsendcells) {
+        CU(cudaMemcpyAsync(c->d_send_cells, c->Z.send_cells.data(), c->nsendcells * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        k_za_mark_send<<<grid_for(c->nsendcells, c->grid_light), 256, 0, c->stream>>>(CO.c2e, c->d_send_cells, (int)c->nsendcells);
+    }
+    // boundary kinds / values follow the tags of the global edges; state, gradient and flux buffers
+    {
+        std::vector<int> ge((size_t)nb);
+        if (nb) CU(cudaMemcpyAsync(ge.data(), d_gedge, (size_t)nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        st.h_btag.assign((size_t)nb, -1);
+        for (long long j = 0; j < nb; ++j) st.h_btag[j] = c->g.h_btag[ge[j] - ne_int_g];
+    }
+    CU(st.alloc(&st.d_bkind, (size_t)nb)); CU(st.alloc(&st.d_bval, (size_t)nb)); CU(st.alloc(&st.d_nman, (size_t)ncz));
+    d.bkind = st.d_bkind; d.bval = st.d_bval; d.nman = st.d_nman;
+    CU(st.alloc(&st.A, (size_t)ncz)); CU(st.alloc(&st.B, (size_t)ncz)); CU(st.alloc(&st.grad, 3 * (size_t)ncz));
+    CU(st.alloc(&st.F.f1, (size_t)nez)); CU(st.alloc(&st.F.fxl, (size_t)nez)); CU(st.alloc(&st.F.fyl, (size_t)nez));
+    CU(st.alloc(&st.F.fxr, (size_t)nez)); CU(st.alloc(&st.F.fyr, (size_t)nez));
+    {
+        const size_t wc = ((size_t)ncz + 31) / 32 + 1, we = ((size_t)nez + 31) / 32 + 1;
+        st.mask_words = 3 * wc + we;
+        CU(st.alloc(&st.zA, st.mask_words));
+        st.zB = st.zA + wc; st.gz = st.zB + wc; st.fz = st.gz + wc;
+    }
+    CU(cudaMemsetAsync(st.grad, 0, 3 * (size_t)ncz * sizeof(double4), c->stream));
+    mark("buffers allocated");
+    // the host's copy of the cell lists is fetched when swe_zone_cells asks for it (zone_cells_to_host)
+    c->zr_zone = zid; c->zr_off = coff;
+    c->zone_ms[4] = ms_since(t0);
     c->nsend = (int64_t)c->Z.send_idx.size();
     const size_t ns = (size_t)(c->nsend ? c->nsend : 1);
     CU(cudaMalloc((void**)&c->d_send_idx, ns * sizeof(int)));
     CU(cudaMalloc((void**)&c->d_recv_idx, ns * sizeof(int)));
-    CU(cudaMalloc((void**)&c->d_src_of_cell, (size_t)c->z.nc * sizeof(int)));
     CU(cudaMalloc((void**)&c->d_sendbuf, ns * 8 * sizeof(double)));
     if (c->nsend) {
         CU(cudaMemcpyAsync(c->d_send_idx, c->Z.send_idx.data(), c->nsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         CU(cudaMemcpyAsync(c->d_recv_idx, c->Z.recv_idx.data(), c->nsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     }
-    CU(cudaMemcpyAsync(c->d_src_of_cell, c->Z.src_of_cell.data(), (size_t)c->z.nc * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     c->nrsend = (int64_t)c->Z.rsend_idx.size();
     c->nrrecv = (int64_t)c->Z.rrecv_idx.size();
     CU(cudaMalloc((void**)&c->d_rsend_idx, (size_t)(c->nrsend ? c->nrsend : 1) * sizeof(int)));
@@ -1139,9 +1434,6 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
         CU(cudaMemcpyAsync(c->d_rsend_dst, c->Z.rsend_dst.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         CU(cudaMemcpyAsync(c->d_rsend_peer, c->Z.rsend_peer.data(), c->nrsend * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     }
-    c->nsendcells = (int64_t)c->Z.send_cells.size();
-    CU(cudaMalloc((void**)&c->d_send_cells, (size_t)(c->nsendcells ? c->nsendcells : 1) * sizeof(int)));
-    if (c->nsendcells) CU(cudaMemcpyAsync(c->d_send_cells, c->Z.send_cells.data(), c->nsendcells * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMalloc((void**)&c->d_peerA, (size_t)nranks * sizeof(double4*)));
     CU(cudaMalloc((void**)&c->d_peerB, (size_t)nranks * sizeof(double4*)));
     c->peerA.assign(nranks, nullptr); c->peerB.assign(nranks, nullptr); c->peer_ipc.assign(nranks, 0);
@@ -1153,8 +1445,6 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     k_gather_scalar<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.d_nman, c->g.d_nman, c->d_src_of_cell, (int)c->z.nc);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(c->stream));
-    // the host copies of the big zoned arrays are no longer needed
-    c->Z.mesh = MeshArrays();
     c->zone_ms[2] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     return SWE_OK;
 }
@@ -1404,7 +1694,7 @@ int swe_zone_stats(const swe_ctx* c, int64_t* send_cells_total, int64_t* bytes_p
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
     int64_t gh = 0;
-    for (const ZoneDesc& zd : c->Z.z) if (zd.offset >= 0) gh += (int64_t)zd.cells.size() - zd.nowned;
+    for (const ZoneDesc& zd : c->Z.z) if (zd.offset >= 0) gh += zd.ncells - zd.nowned;
     if (send_cells_total) *send_cells_total = c->nsend;
     if (bytes_per_exchange) *bytes_per_exchange = c->nsend * 24;
     if (ghost_cells_total) *ghost_cells_total = gh;
@@ -1418,18 +1708,49 @@ int swe_zone_setup_ms(const swe_ctx* c, double* ghost_layers_ms, double* build_m
     if (total_ms) *total_ms = c->zone_ms[2];
     return SWE_OK;
 }
+int swe_zone_setup_detail(const swe_ctx* c, double* ms /*5*/) {
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!c->has_zones) return fail(SWE_ERR_STATE, "no zones");
+    if (!ms) return fail(SWE_ERR_ARG, "NULL output");
+    ms[0] = c->zone_ms[3];                      // zone of every cell (RCB or the caller's array)
+    ms[1] = c->zone_ms[0];                      // ghost layers of all zones on the device
+    ms[2] = c->zone_ms[1] - c->zone_ms[3] - c->zone_ms[0];   // owned positions (device) + links and exchange lists (host)
+    ms[3] = c->zone_ms[4] - c->zone_ms[1];      // the zones' arrays assembled on the device
+    ms[4] = c->zone_ms[2];                      // whole call
+    return SWE_OK;
+}
 int swe_zone_describe(const swe_ctx* c, int zone, int64_t* nowned, int64_t* nghost, int64_t* nlinks) {
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
     const ZoneDesc& zd = c->Z.z[zone];
     if (nowned) *nowned = zd.nowned;
-    if (nghost) *nghost = (int64_t)zd.cells.size() - zd.nowned;
+    if (nghost) *nghost = zd.ncells - zd.nowned;
     if (nlinks) *nlinks = (int64_t)zd.links.size();
     return SWE_OK;
 }
-int swe_zone_cells(const swe_ctx* c, int zone, int32_t* cells, int32_t* layer) {
+// the zones' cell lists (source cell and layer of every cell of the concatenated mesh): one download,
+// sliced per resident zone, the first time somebody asks
+static int zone_cells_to_host(swe_ctx* c) {
+    if (c->zone_cells_on_host) return SWE_OK;
+    const size_t ncz = (size_t)c->z.nc;
+    std::vector<int32_t> hsrc(ncz); std::vector<uint8_t> hlay(ncz);
+    CU(cudaMemcpyAsync(hsrc.data(), c->d_src_of_cell, ncz * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(hlay.data(), c->z.dm.layer, ncz, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    for (size_t r = 0; r < c->zr_zone.size(); ++r) {
+        ZoneDesc& zd = c->Z.z[c->zr_zone[r]];
+        zd.cells.assign(hsrc.begin() + c->zr_off[r], hsrc.begin() + c->zr_off[r] + zd.ncells);
+        zd.layer.assign(hlay.begin() + c->zr_off[r], hlay.begin() + c->zr_off[r] + zd.ncells);
+    }
+    c->zone_cells_on_host = true;
+    return SWE_OK;
+}
+int swe_zone_cells(const swe_ctx* cc, int zone, int32_t* cells, int32_t* layer) {
+    swe_ctx* c = const_cast<swe_ctx*>(cc);
     if (check_ctx(c)) return SWE_ERR_ARG;
     if (!c->has_zones || zone < 0 || zone >= c->Z.nz) return fail(SWE_ERR_ARG, "no such zone");
+    if (c->Z.zone_rank[zone] != c->Z.rank) return fail(SWE_ERR_ARG, "the zone lives on another rank");
+    { int rc = zone_cells_to_host(c); if (rc) return rc; }
     const ZoneDesc& zd = c->Z.z[zone];
     for (size_t j = 0; j < zd.cells.size(); ++j) {
         if (cells) cells[j] = c->H.m.cell_user[zd.cells[j]];

@@ -115,9 +115,13 @@ __global__ void __launch_bounds__(1024) k_rs_scan(unsigned int* __restrict__ his
 // stable scatter: the tile is walked in rounds of 256 consecutive keys; inside a round the rank of
 // a key among the equal digits before it comes from __match_any_sync (within the warp) and the
 // per-warp digit counts (across the warps of the block)
+// VAL: a 32-bit value travels with every key (vin -> vout)
+template <bool VAL>
 __global__ void __launch_bounds__(RS_THREADS) k_rs_scatter(const unsigned long long* __restrict__ in,
                                                            unsigned long long* __restrict__ out, long long n, int shift,
-                                                           const unsigned int* __restrict__ hist, int nblk) {
+                                                           const unsigned int* __restrict__ hist, int nblk,
+                                                           const unsigned int* __restrict__ vin = nullptr,
+                                                           unsigned int* __restrict__ vout = nullptr) {
     __shared__ unsigned int base[256];
     __shared__ unsigned int wcnt[RS_THREADS / 32][256];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -139,6 +143,7 @@ __global__ void __launch_bounds__(RS_THREADS) k_rs_scatter(const unsigned long l
             unsigned int off = base[d] + rank;
             for (int w = 0; w < wid; ++w) off += wcnt[w][d];
             out[off] = key;
+            if (VAL) vout[off] = vin[i];
         }
         __syncthreads();
         unsigned int tot = 0;
