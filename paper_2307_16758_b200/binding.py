@@ -446,7 +446,7 @@ def create_from_config(cfg, renumber=SWE_RENUM_HILBERT, cuda_stream=None):
 
 
 # ---- host-only inspection (no GPU) ----------------------------------------------------------
-_HOST_DTYPES = {"eside": np.uint8, "cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": np.int32, "btag": np.int32,
+_HOST_DTYPES = {"eside": np.uint8, "rres": np.float32, "cell_user": np.int32, "c2c": np.int32, "c2e": np.int32, "elr": np.int32, "btag": np.int32,
                 "user_cell": np.int32, "zone_of": np.int32, "send_idx": np.int32, "recv_idx": np.int32,
                 "src_of_cell": np.int32, "link_src": np.int32, "link_dst": np.int32, "tags": np.int32,
                 "zone_rank": np.int32, "rsend_idx": np.int32, "rsend_dst": np.int32, "rsend_peer": np.int32,

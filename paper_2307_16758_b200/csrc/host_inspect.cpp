@@ -35,6 +35,7 @@ int64_t mesh_get(const MeshArrays& M, const std::string& n, void* out, int64_t c
     if (n == "r0") return copy_out(M.r[0], out, cap);
     if (n == "r1") return copy_out(M.r[1], out, cap);
     if (n == "r2") return copy_out(M.r[2], out, cap);
+    if (n == "rres") return copy_out(M.rres, out, cap);
     if (n == "elr") return copy_out(M.elr, out, cap);
     if (n == "en") return copy_out(M.en, out, cap);
     if (n == "elen") return copy_out(M.elen, out, cap);

@@ -260,6 +260,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
     M.c2c.assign(4 * nt, 0); M.c2e.assign(4 * nt, 0);
     M.zc.resize(nt); M.area.resize(nt); M.rin.resize(nt);
     for (int k = 0; k < 3; ++k) { M.w[k].resize(2 * nt); M.r[k].resize(2 * nt); }
+    M.rres.resize(2 * nt);
     M.elr.resize(2 * ne); M.en.resize(2 * ne); M.elen.resize(ne); M.edx.resize(ne);
     M.erl.resize(2 * ne); M.err.resize(2 * ne);
     M.btag.assign(nbe, -1);
@@ -302,6 +303,8 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
             }
             M.r[k][2 * i] = rx[k]; M.r[k][2 * i + 1] = ry[k];
         }
+        for (int q = 0; q < 2; ++q)                           // residual of r_0 + r_1 + r_2 = 0 (exact in double: the sum cancels)
+            M.rres[2 * i + q] = (float)(M.r[2][2 * i + q] + (M.r[0][2 * i + q] + M.r[1][2 * i + q]));
         M.rin[i] = 2.0 * area[u] / (lk[0] + lk[1] + lk[2]);   // A.1.5
         min_rin = std::min(min_rin, M.rin[i]);
         // A.1.7: w_k = N^-1 d_k with the normal matrix N = sum_k d_k d_k^T of the three stencil
@@ -529,6 +532,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     M.cell_user.resize(ncz); M.c2c.assign(4 * ncz, 0); M.c2e.assign(4 * ncz, 0);
     M.zc.resize(ncz); M.area.resize(ncz); M.rin.resize(ncz);
     for (int k = 0; k < 3; ++k) { M.w[k].resize(2 * ncz); M.r[k].resize(2 * ncz); }
+    M.rres.resize(2 * ncz);
     Z.src_of_cell.resize(ncz);
     std::vector<int32_t> loc(nc, -1);
     std::vector<int32_t> emark(G.ne, -1);
@@ -597,6 +601,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             Z.src_of_cell[c] = (int32_t)g;
             M.zc[c] = G.zc[g]; M.area[c] = G.area[g]; M.rin[c] = G.rin[g];
             for (int k = 0; k < 3; ++k) M.dupw[4 * c + k] = G.dupw[4 * g + k];
+            M.rres[2 * c] = G.rres[2 * g]; M.rres[2 * c + 1] = G.rres[2 * g + 1];
             for (int k = 0; k < 3; ++k) {
                 M.w[k][2 * c] = G.w[k][2 * g]; M.w[k][2 * c + 1] = G.w[k][2 * g + 1];
                 M.r[k][2 * c] = G.r[k][2 * g]; M.r[k][2 * c + 1] = G.r[k][2 * g + 1];

@@ -24,6 +24,8 @@ struct MeshArrays {
     std::vector<double> zc, area, rin;       // cell bed, |Omega_i|, in-radius
     std::vector<double> w[3];                // 2*nc each: least-squares weights (wx,wy) of side k
     std::vector<double> r[3];                // 2*nc each: r_{i,k} = m_e - c_i
+    std::vector<float> rres;                 // 2*nc: r_{i,2} + (r_{i,0} + r_{i,1}) in single precision (the device
+                                             //       stores r_0, r_1 and this instead of r_2: swe_kernels.cuh stencil_r2)
     std::vector<double> dupw;                // 4*nc: |x_i - x_upw| for side 0,1,2 (multislope MUSCL), pad
     // per edge
     std::vector<int32_t> elr;                // 2*ne: L cell, R cell (-1 on the boundary)

@@ -42,6 +42,7 @@ struct Store {
     int* d_bkind = nullptr;
     double* d_bval = nullptr;
     double* d_nman = nullptr;
+    int4* d_c2e = nullptr;             // = dm.c2e, writable (Manning codes in c2e.w)
     std::vector<int32_t> h_btag;
     double4 *A = nullptr, *B = nullptr, *grad = nullptr;
     FluxBuf F{};
@@ -92,6 +93,8 @@ struct swe_ctx {
     double beta = 1.0;
     std::map<int, std::pair<int, double>> bc;
     StepScalars* d_S = nullptr;
+    double* d_nman_tab = nullptr;      // 256 doubles: Manning n by code (c2e.w bits 8-15)
+    unsigned char* d_ncode = nullptr;  // per USER cell, kept for zones created later
     int* d_flag = nullptr;             // validation flag of swe_set_state
     bool min_valid = false;
     int64_t launches = 0, halo_bytes = 0, steps = 0;
@@ -209,12 +212,19 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.upload(&area, M.area.data(), (size_t)M.nc, s));
     CU(st.upload(&rin, M.rin.data(), (size_t)M.nc, s));
     d.c2c = c2c; d.c2e = c2e; d.zc = zc; d.area = area; d.rin = rin;
+    st.d_c2e = c2e;
     for (int k = 0; k < 3; ++k) {
-        double2 *w, *r;
+        double2 *w, *r = nullptr;
         CU(st.upload(&w, M.w[k].data(), (size_t)M.nc, s));
-        CU(st.upload(&r, M.r[k].data(), (size_t)M.nc, s));
+        if (k < 2) CU(st.upload(&r, M.r[k].data(), (size_t)M.nc, s));      // r_2 travels as the residual rres
         d.w[k] = w; d.r[k] = r;
     }
+    {
+        float2* rres;
+        CU(st.upload(&rres, M.rres.data(), (size_t)M.nc, s));
+        d.rres = rres;
+    }
+    d.nman_tab = c->d_nman_tab;
     int2* elr; double2 *en, *erl, *err; double *elen, *edx;
     CU(st.upload(&elr, M.elr.data(), (size_t)M.ne, s));
     CU(st.upload(&en, M.en.data(), (size_t)M.ne, s));
@@ -533,7 +543,15 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     c->grid_flux[K_MUSCL_MS] = occ((const void*)k_edge_flux<K_MUSCL_MS, false>, 2, SWE_FLUX_THREADS);
     c->grid_upd = occ((const void*)k_cell_update<1, true, false>, 4);
     c->grid_ms = occ((const void*)k_ms_slopes, 5, 128);
-    int rc = upload_store(c, c->g, c->H.m);
+    int rc = SWE_OK;
+    {
+        cudaError_t e = cudaMalloc((void**)&c->d_nman_tab, 256 * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_nman_tab, 0, 256 * sizeof(double), c->stream);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&c->d_ncode, (size_t)c->H.nt);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_ncode, 0, (size_t)c->H.nt, c->stream);
+        if (e != cudaSuccess) rc = fail(SWE_ERR_CUDA, cudaGetErrorString(e));
+    }
+    if (rc == SWE_OK) rc = upload_store(c, c->g, c->H.m);
     if (rc == SWE_OK) {
         cudaError_t e = cudaMalloc((void**)&c->d_S, sizeof(StepScalars));
         if (e == cudaSuccess) e = cudaMalloc((void**)&c->d_flag, sizeof(int));
@@ -570,6 +588,8 @@ int swe_mesh_destroy(swe_ctx* c) {
     if (c->d_S) cudaFree(c->d_S);
     if (c->d_flag) cudaFree(c->d_flag);
     if (c->d_stage) cudaFree(c->d_stage);
+    if (c->d_nman_tab) cudaFree(c->d_nman_tab);
+    if (c->d_ncode) cudaFree(c->d_ncode);
     delete c;
     return SWE_OK;
 }
@@ -615,6 +635,43 @@ int swe_set_manning(swe_ctx* c, const double* n_cell) {
     }
     if (c->has_zones) {
         k_gather_scalar<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.d_nman, c->g.d_nman, c->d_src_of_cell, (int)c->z.nc);
+        CU(cudaGetLastError());
+    }
+    // the distinct values as a table, a one-byte code per cell in c2e.w (swe_kernels.cuh c2e_ncode):
+    // the update kernel then reads nothing per cell for n.  More than 255 distinct values: code 255
+    // everywhere, the kernel reads the array.
+    {
+        std::vector<double> hn;
+        const double* hv = n_cell;
+        if (n_cell && is_device_ptr(n_cell)) {
+            hn.resize((size_t)nt);
+            CU(cudaMemcpyAsync(hn.data(), n_cell, nt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            hv = hn.data();
+        }
+        std::vector<unsigned char> code((size_t)nt, 0);
+        std::vector<double> tab(256, 0.0);
+        bool fits = true;
+        if (hv) {
+            std::vector<uint64_t> bits;                       // the table, by bit pattern
+            int last = -1;
+            for (int64_t i = 0; i < nt && fits; ++i) {
+                uint64_t b; std::memcpy(&b, &hv[i], 8);
+                int k = (last >= 0 && bits[last] == b) ? last : -1;
+                for (int j = 0; k < 0 && j < (int)bits.size(); ++j) if (bits[j] == b) k = j;
+                if (k < 0) {
+                    if (bits.size() == 255) { fits = false; break; }
+                    k = (int)bits.size(); bits.push_back(b); tab[k] = hv[i];
+                }
+                code[i] = (unsigned char)k; last = k;
+            }
+        }
+        if (!fits) std::fill(code.begin(), code.end(), (unsigned char)255);
+        CU(cudaMemcpyAsync(c->d_nman_tab, tab.data(), 256 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_ncode, code.data(), (size_t)nt, cudaMemcpyHostToDevice, c->stream));
+        k_set_ncode<<<grid_for(nt, c->grid_light), 256, 0, c->stream>>>(c->g.d_c2e, c->g.d_cell_user, c->d_ncode, (int)nt);
+        if (c->has_zones)
+            k_set_ncode<<<grid_for(c->z.nc, c->grid_light), 256, 0, c->stream>>>(c->z.d_c2e, c->z.d_cell_user, c->d_ncode, (int)c->z.nc);
         CU(cudaGetLastError());
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -1362,7 +1419,8 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     CU(st.alloc(&CO.c2c, (size_t)ncz)); CU(st.alloc(&CO.c2e, (size_t)ncz)); CU(st.alloc(&CO.cell_user, (size_t)ncz));
     CU(st.alloc(&CO.zc, (size_t)ncz)); CU(st.alloc(&CO.area, (size_t)ncz)); CU(st.alloc(&CO.rin, (size_t)ncz));
     CU(st.alloc(&CO.dupw, (size_t)ncz));
-    for (int k = 0; k < 3; ++k) { CU(st.alloc(&CO.w[k], (size_t)ncz)); CU(st.alloc(&CO.r[k], (size_t)ncz)); }
+    for (int k = 0; k < 3; ++k) CU(st.alloc(&CO.w[k], (size_t)ncz));
+    CU(st.alloc(&CO.r[0], (size_t)ncz)); CU(st.alloc(&CO.r[1], (size_t)ncz)); CU(st.alloc(&CO.rres, (size_t)ncz));
     CU(st.alloc(&EO.elr, (size_t)nez)); CU(st.alloc(&EO.en, (size_t)nez)); CU(st.alloc(&EO.elen, (size_t)nez));
     CU(st.alloc(&EO.edx, (size_t)nez)); CU(st.alloc(&EO.erl, (size_t)nez)); CU(st.alloc(&EO.err, (size_t)nez));
     CU(st.alloc(&EO.edlr, (size_t)nez)); CU(st.alloc(&EO.ernorm, (size_t)nez)); CU(st.alloc(&EO.eside, (size_t)nez));
@@ -1376,7 +1434,10 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     c->launches += 7;
     CU(cudaGetLastError());
     d.c2c = CO.c2c; d.c2e = CO.c2e; d.zc = CO.zc; d.area = CO.area; d.rin = CO.rin; d.dupw = CO.dupw;
-    for (int k = 0; k < 3; ++k) { d.w[k] = CO.w[k]; d.r[k] = CO.r[k]; }
+    for (int k = 0; k < 3; ++k) d.w[k] = CO.w[k];
+    d.r[0] = CO.r[0]; d.r[1] = CO.r[1]; d.r[2] = nullptr; d.rres = CO.rres;
+    d.nman_tab = c->d_nman_tab;
+    st.d_c2e = CO.c2e;
     d.elr = EO.elr; d.en = EO.en; d.elen = EO.elen; d.edx = EO.edx; d.erl = EO.erl; d.err = EO.err;
     d.edlr = EO.edlr; d.ernorm = EO.ernorm; d.eside = EO.eside;
     d.layer = d_lay;

@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(256) k_za_bnd_edges(ZoneTabs T, const int* __r
 // ---- fill: per-cell arrays of the concatenated mesh ----
 struct ZoneCellOut {
     int4* c2c; int4* c2e; int* cell_user; double* zc; double* area; double* rin; double4* dupw;
-    double2* w[3]; double2* r[3];
+    double2* w[3]; double2* r[2]; float2* rres;
 };
 __global__ void __launch_bounds__(256) k_za_fill_cells(ZoneTabs T, DevMesh G, const int* __restrict__ g_cell_user,
                                                        const int* __restrict__ zone_of, const int* __restrict__ owned_pos,
@@ -212,7 +212,8 @@ __global__ void __launch_bounds__(256) k_za_fill_cells(ZoneTabs T, DevMesh G, co
         O.cell_user[c] = g_cell_user[g];
         O.zc[c] = G.zc[g]; O.area[c] = G.area[g]; O.rin[c] = G.rin[g]; O.dupw[c] = G.dupw[g];
         #pragma unroll
-        for (int k = 0; k < 3; ++k) { O.w[k][c] = G.w[k][g]; O.r[k][c] = G.r[k][g]; }
+        for (int k = 0; k < 3; ++k) O.w[k][c] = G.w[k][g];
+        O.r[0][c] = G.r[0][g]; O.r[1][c] = G.r[1][g]; O.rres[c] = G.rres[g];
         const int4 nb = G.c2c[g], ce = G.c2e[g];
         const int nk[3] = {nb.x, nb.y, nb.z}, ek[3] = {ce.x, ce.y, ce.z};
         int on[3], oe[3];
@@ -234,11 +235,11 @@ __global__ void __launch_bounds__(256) k_za_fill_cells(ZoneTabs T, DevMesh G, co
             }
         }
         O.c2c[c] = make_int4(on[0], on[1], on[2], lay);
-        O.c2e[c] = make_int4(oe[0], oe[1], oe[2], lay);
+        O.c2e[c] = make_int4(oe[0], oe[1], oe[2], lay | (ce.w & 0xff00));      // the cell's Manning code travels along
     }
 }
 __global__ void __launch_bounds__(256) k_za_mark_send(int4* __restrict__ c2e, const int* __restrict__ cells, int n) {
-    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) c2e[cells[j]].w = -1;
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) c2e[cells[j]].w |= 0xff;   // flag -1, Manning code kept
 }
 
 // ---- fill: per-edge arrays (d < ne_int_z: interior edge ikeys[d]; else boundary edge bkeys[d - ne_int_z]) ----

@@ -238,3 +238,30 @@ def test_rcm_order_has_a_small_bandwidth():
     assert bw[sw.SWE_RENUM_NONE][0] > nt // 2
     assert bw[sw.SWE_RENUM_RCM][0] < 6 * 60                  # a few rows of the 60 x 60 x 2 mesh
     assert bw[sw.SWE_RENUM_RCM][1] < 0.05 * bw[sw.SWE_RENUM_NONE][1]
+
+
+def test_third_offset_travels_as_a_single_precision_residual():
+    """The device stores r_0, r_1 and rres = float(r_2 + (r_0 + r_1)) instead of r_2 (8 bytes less
+    per cell and stage in the gradient kernel; swe_kernels.cuh stencil_r2): the reconstruction
+    rres - (r_0 + r_1) must give back the stored r_2 -- bit for bit except where a component of r_2
+    is tiny against |r| (there within an ulp of |r|) -- on meshes with coordinates up to 6e4 m."""
+    for cfg in (config3(length=3200.0, half_width=600.0, w2=30.0, n4=4, n8=3), config1(n=60),
+                delaunay_case(n=1500)):
+        shift = dict(cfg)
+        shift["x"] = cfg["x"] + 56000.0                     # the far end of the 60 km reach
+        for c in (cfg, shift):
+            h = sw.swe_host_mesh_build(c["x"], c["y"], c["zb"], c["tri"], c["bedge"], c["btag"])
+            try:
+                r0, r1, r2 = [sw.swe_host_get(h, k).reshape(-1, 2) for k in ("r0", "r1", "r2")]
+                res = sw.swe_host_get(h, "rres").reshape(-1, 2)
+                assert res.dtype == np.float32
+                exact = r2 + (r0 + r1)                          # the sum cancels: exact in double
+                assert np.array_equal(res, exact.astype(np.float32))
+                back = res.astype(np.float64) - (r0 + r1)
+                scale = np.sqrt((r2 ** 2).sum(axis=1, keepdims=True))
+                assert np.abs(back - r2).max() <= 1.2e-16 * scale.max()
+                big = np.abs(r2) > 1e-2 * scale
+                assert np.array_equal(back[big], r2[big])
+                assert (back == r2).mean() > 0.999
+            finally:
+                sw.swe_host_mesh_free(h)
