@@ -39,6 +39,7 @@ int64_t mesh_get(const MeshArrays& M, const std::string& n, void* out, int64_t c
     if (n == "elr") return copy_out(M.elr, out, cap);
     if (n == "en") return copy_out(M.en, out, cap);
     if (n == "elen") return copy_out(M.elen, out, cap);
+    if (n == "ed") return copy_out(M.ed, out, cap);
     if (n == "edx") return copy_out(M.edx, out, cap);
     if (n == "erl") return copy_out(M.erl, out, cap);
     if (n == "err") return copy_out(M.err, out, cap);

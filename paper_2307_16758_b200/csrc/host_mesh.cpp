@@ -107,7 +107,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
     const int64_t ne = (int64_t)esL.size();
 
     // ---- A.1.4 / A.1.6 : edge geometry from the end points a->b as traversed by the L-cell ----
-    std::vector<double> elen(ne), enx(ne), eny(ne), edx(ne), rlx(ne), rly(ne), rrx(ne), rry(ne);
+    std::vector<double> elen(ne), enx(ne), eny(ne), edx(ne), rlx(ne), rly(ne), rrx(ne), rry(ne), evx(ne), evy(ne);
     std::vector<int32_t> utag(ne, -1);
     int64_t nbe = 0;
     for (int64_t e = 0; e < ne; ++e) {
@@ -118,6 +118,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         double n1 = dy / len, n2 = -dx / len;
         double mx = 0.5 * (x[a] + x[b]), my = 0.5 * (y[a] + y[b]);
         elen[e] = len; enx[e] = n1; eny[e] = n2;
+        evx[e] = dy; evy[e] = -dx;
         rlx[e] = mx - ucx[L]; rly[e] = my - ucy[L];
         if (esR[e] >= 0) {
             int64_t R = esR[e] / 3;
@@ -262,7 +263,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
     for (int k = 0; k < 3; ++k) { M.w[k].resize(2 * nt); M.r[k].resize(2 * nt); }
     M.rres.resize(2 * nt);
     M.elr.resize(2 * ne); M.en.resize(2 * ne); M.elen.resize(ne); M.edx.resize(ne);
-    M.erl.resize(2 * ne); M.err.resize(2 * ne);
+    M.erl.resize(2 * ne); M.err.resize(2 * ne); M.ed.resize(2 * ne);
     M.btag.assign(nbe, -1);
     H.cx.resize(nt); H.cy.resize(nt);
     for (int64_t d = 0; d < ne; ++d) {
@@ -271,6 +272,7 @@ bool build_host_mesh(HostMesh& H, int64_t nv, const double* x, const double* y, 
         M.elr[2 * d + 1] = esR[e] >= 0 ? H.user_cell[esR[e] / 3] : -1;
         M.en[2 * d] = enx[e]; M.en[2 * d + 1] = eny[e];
         M.elen[d] = elen[e]; M.edx[d] = edx[e];
+        M.ed[2 * d] = evx[e]; M.ed[2 * d + 1] = evy[e];
         M.erl[2 * d] = rlx[e]; M.erl[2 * d + 1] = rly[e];
         M.err[2 * d] = rrx[e]; M.err[2 * d + 1] = rry[e];
         if (d >= M.ne_int) M.btag[d - M.ne_int] = utag[e];
@@ -568,7 +570,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
     if (M.ne > (int64_t)INT32_MAX / 2) { err = "zoned mesh too large"; return false; }
     M.elr.resize(2 * M.ne); M.en.resize(2 * M.ne); M.elen.resize(M.ne); M.edx.resize(M.ne);
     M.erl.resize(2 * M.ne); M.err.resize(2 * M.ne); M.edlr.resize(M.ne);
-    M.eside.resize(M.ne); M.ernorm.resize(2 * M.ne);
+    M.eside.resize(M.ne); M.ernorm.resize(2 * M.ne); M.ed.resize(2 * M.ne);
     M.dupw.assign(4 * (size_t)ncz, 0.0);
     M.btag.assign(M.ne - M.ne_int, -1);
     std::vector<int32_t> eloc(G.ne, -1);
@@ -582,6 +584,7 @@ bool build_zones(const HostMesh& H, ZoneSet& Z, int nz, int nlayers, const int32
             M.elr[2 * d] = (int32_t)(o + loc[L]);
             M.elr[2 * d + 1] = R >= 0 ? (int32_t)(o + loc[R]) : -1;
             M.en[2 * d] = G.en[2 * (int64_t)e]; M.en[2 * d + 1] = G.en[2 * (int64_t)e + 1];
+            M.ed[2 * d] = G.ed[2 * (int64_t)e]; M.ed[2 * d + 1] = G.ed[2 * (int64_t)e + 1];
             M.elen[d] = G.elen[e]; M.edx[d] = G.edx[e]; M.edlr[d] = G.edlr[e]; M.eside[d] = G.eside[e];
             M.ernorm[2 * d] = G.ernorm[2 * (int64_t)e]; M.ernorm[2 * d + 1] = G.ernorm[2 * (int64_t)e + 1];
             M.erl[2 * d] = G.erl[2 * (int64_t)e]; M.erl[2 * d + 1] = G.erl[2 * (int64_t)e + 1];

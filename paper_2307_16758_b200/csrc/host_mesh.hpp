@@ -31,6 +31,7 @@ struct MeshArrays {
     std::vector<int32_t> elr;                // 2*ne: L cell, R cell (-1 on the boundary)
     std::vector<double> en;                  // 2*ne: unit normal, outward of L
     std::vector<double> elen, edx;           // length, WAF Delta-x
+    std::vector<double> ed;                  // 2*ne: (dy, -dx) of the edge along its L-cell: en = ed / elen, elen = |ed|
     std::vector<double> erl, err;            // 2*ne each: r_{L,e}, r_{R,e}
     std::vector<double> edlr;                // |x_R - x_L| between the centroids (0 on the boundary)
     std::vector<double> ernorm;              // 2*ne: |r_{L,e}|, |r_{R,e}| (multislope MUSCL face distances)

@@ -233,6 +233,11 @@ int upload_store(swe_ctx* c, Store& st, const MeshArrays& M) {
     CU(st.upload(&erl, M.erl.data(), (size_t)M.ne, s));
     CU(st.upload(&err, M.err.data(), (size_t)M.ne, s));
     d.elr = elr; d.en = en; d.elen = elen; d.edx = edx; d.erl = erl; d.err = err;
+    {
+        double2* ed;
+        CU(st.upload(&ed, M.ed.data(), (size_t)M.ne, s));
+        d.ed = ed;
+    }
     double4* dupw; double* edlr; uint8_t* eside;
     CU(st.upload(&dupw, M.dupw.data(), (size_t)M.nc, s));
     CU(st.upload(&edlr, M.edlr.data(), (size_t)M.ne, s));
@@ -1424,6 +1429,7 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     CU(st.alloc(&EO.elr, (size_t)nez)); CU(st.alloc(&EO.en, (size_t)nez)); CU(st.alloc(&EO.elen, (size_t)nez));
     CU(st.alloc(&EO.edx, (size_t)nez)); CU(st.alloc(&EO.erl, (size_t)nez)); CU(st.alloc(&EO.err, (size_t)nez));
     CU(st.alloc(&EO.edlr, (size_t)nez)); CU(st.alloc(&EO.ernorm, (size_t)nez)); CU(st.alloc(&EO.eside, (size_t)nez));
+    CU(st.alloc(&EO.ed, (size_t)nez));
     int* d_gedge = nullptr;
     CU(tmp.get(&d_gedge, (size_t)nb));
     EO.gedge = d_gedge;
@@ -1439,7 +1445,7 @@ static int zones_create_impl(swe_ctx* c, int nzones, int nlayers, const int32_t*
     d.nman_tab = c->d_nman_tab;
     st.d_c2e = CO.c2e;
     d.elr = EO.elr; d.en = EO.en; d.elen = EO.elen; d.edx = EO.edx; d.erl = EO.erl; d.err = EO.err;
-    d.edlr = EO.edlr; d.ernorm = EO.ernorm; d.eside = EO.eside;
+    d.edlr = EO.edlr; d.ernorm = EO.ernorm; d.eside = EO.eside; d.ed = EO.ed;
     d.layer = d_lay;
     st.d_cell_user = CO.cell_user;
     mark("arrays filled");

@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(256) k_za_mark_send(int4* __restrict__ c2e, co
 
 // ---- fill: per-edge arrays (d < ne_int_z: interior edge ikeys[d]; else boundary edge bkeys[d - ne_int_z]) ----
 struct ZoneEdgeOut {
-    int2* elr; double2* en; double* elen; double* edx; double2* erl; double2* err; double* edlr; double2* ernorm;
+    int2* elr; double2* en; double2* ed; double* elen; double* edx; double2* erl; double2* err; double* edlr; double2* ernorm;
     uint8_t* eside; int* gedge;      // gedge: global id of every boundary edge (for the tags), [ne_z - ne_int_z]
 };
 __global__ void __launch_bounds__(256) k_za_fill_edges(ZoneTabs T, DevMesh G, const int* __restrict__ zone_of,
@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(256) k_za_fill_edges(ZoneTabs T, DevMesh G, co
         const int2 lr = G.elr[e];
         O.elr[d] = make_int2(za_loc(T, zone_of, owned_pos, gkeys, r, lr.x),
                              lr.y >= 0 ? za_loc(T, zone_of, owned_pos, gkeys, r, lr.y) : -1);
-        O.en[d] = G.en[e]; O.elen[d] = G.elen[e]; O.edx[d] = G.edx[e]; O.erl[d] = G.erl[e]; O.err[d] = G.err[e];
+        O.en[d] = G.en[e]; O.ed[d] = G.ed[e]; O.elen[d] = G.elen[e]; O.edx[d] = G.edx[e]; O.erl[d] = G.erl[e]; O.err[d] = G.err[e];
         O.edlr[d] = G.edlr[e]; O.ernorm[d] = G.ernorm[e]; O.eside[d] = G.eside[e];
         if (d >= ne_int_z) O.gedge[d - ne_int_z] = e;
     }
