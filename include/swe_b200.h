@@ -87,6 +87,23 @@ int swe_set_bc(swe_ctx* ctx, int tag, int kind, double value);
  * left as it was).  The simulated time t is not touched; use swe_set_time. */
 int swe_set_state(swe_ctx* ctx, const double* h, const double* hu, const double* hv);
 int swe_get_state(const swe_ctx* ctx, double* h, double* hu, double* hv);
+/* swe_get_state for callers that must not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same result -- h, hu, hv of every cell, user order,
+ * host or device pointers -- but host arrays are staged through a file-scope static device array
+ * of 3 x SWE_STATIC_MAX_CELLS doubles (6 MiB, held by every GPU that loads the library until the
+ * process exits) instead of a buffer that swe_get_state cudaMallocs on first use.  The call makes
+ * no cudaMalloc / cudaFree and calls no allocating library routine; it launches the same kernel
+ * on the context's stream and synchronises that stream before returning.  The device address of the
+ * array is looked up once per device in swe_mesh_create (cudaGetSymbolAddress, with that device
+ * current); the context's device must be current here too.
+ * Limits: meshes of more than SWE_STATIC_MAX_CELLS cells are refused (SWE_ERR_ARG, message names
+ * both numbers).  EVERY context on a device shares the one array and it keeps the last call's
+ * contents: every slot a call copies out it has written first, so nothing needs clearing, but two
+ * calls that overlap on the GPU (two contexts on different streams, two host threads) race on it --
+ * serialise them.  Errors: SWE_ERR_ARG (NULL array, mesh too large), SWE_ERR_STATE (another device
+ * is current), SWE_ERR_CUDA (no device address for the array; a CUDA failure). */
+#define SWE_STATIC_MAX_CELLS 262144
+int swe_get_state_static(const swe_ctx* ctx, double* h, double* hu, double* hv);
 int swe_set_time(swe_ctx* ctx, double t);
 /* Advance nsteps time steps: per step dt = cfl * min_i R_i/lambda_i (eq. 5) by a device
  * min-reduction, then the scheme's stage(s).  Asynchronous on the context's stream (dt never

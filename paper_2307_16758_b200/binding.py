@@ -17,6 +17,7 @@ SWE_ERR_ARG, SWE_ERR_MESH, SWE_ERR_CUDA, SWE_ERR_STATE, SWE_ERR_NOMEM = -1, -2, 
 SWE_HLLC, SWE_MUSCL, SWE_WAF, SWE_MUSCL_MS = 0, 1, 2, 3
 SWE_BC_WALL, SWE_BC_INFLOW_Q, SWE_BC_LEVEL, SWE_BC_TRANSMISSIVE = 0, 1, 2, 3
 SWE_RENUM_NONE, SWE_RENUM_HILBERT, SWE_RENUM_RCM = 0, 1, 2
+SWE_STATIC_MAX_CELLS = 262144      # include/swe_b200.h: the most cells swe_get_state_static serves
 SCHEMES = {"hllc": SWE_HLLC, "muscl": SWE_MUSCL, "waf": SWE_WAF, "muscl_ms": SWE_MUSCL_MS}
 BC_KINDS = {"wall": SWE_BC_WALL, "inflow": SWE_BC_INFLOW_Q, "level": SWE_BC_LEVEL,
             "transmissive": SWE_BC_TRANSMISSIVE}
@@ -35,6 +36,7 @@ SIGNATURES = {
     "swe_set_bc": (C.c_int, [_vp, C.c_int, C.c_int, C.c_double]),
     "swe_set_state": (C.c_int, [_vp, _vp, _vp, _vp]),
     "swe_get_state": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "swe_get_state_static": (C.c_int, [_vp, _vp, _vp, _vp]),
     "swe_set_time": (C.c_int, [_vp, C.c_double]),
     "swe_step": (C.c_int, [_vp, C.c_int, C.c_double, C.c_int, _dp, _dp]),
     "swe_set_graphs": (C.c_int, [_vp, C.c_int]),
@@ -190,6 +192,16 @@ def swe_get_state(ctx, h=None, hu=None, hv=None):
         n = swe_mesh_info(ctx)["ncell"]
         h, hu, hv = np.empty(n), np.empty(n), np.empty(n)
     _check(lib().swe_get_state(ctx, _ptr(h), _ptr(hu), _ptr(hv)))
+    return h, hu, hv
+
+
+def swe_get_state_static(ctx, h=None, hu=None, hv=None):
+    """swe_get_state without any allocation in the library: host arrays are staged through a static
+    device array (meshes of up to SWE_STATIC_MAX_CELLS cells; see include/swe_b200.h)."""
+    if h is None:
+        n = swe_mesh_info(ctx)["ncell"]
+        h, hu, hv = np.empty(n), np.empty(n), np.empty(n)
+    _check(lib().swe_get_state_static(ctx, _ptr(h), _ptr(hu), _ptr(hv)))
     return h, hu, hv
 
 

@@ -80,10 +80,37 @@ struct Scratch {
     ~Scratch() { for (void* v : p) cudaFree(v); }
 };
 
+// ---- swe_get_state_static: staging without an allocation ------------------------------------
+// swe_get_state with host arrays stages the three fields through a device buffer that
+// ensure_stage() cudaMallocs on first use.  Callers that must not allocate (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc) get the same read-back through
+// this file-scope array instead: 3 x SWE_STATIC_MAX_CELLS doubles = 6 MiB, held by every GPU that
+// loads the library until the process exits.  In HOST code the name g_static_stage is a host-side
+// stand-in, not a device address: the address a kernel may use is asked for once per device, with
+// that device current, by cudaGetSymbolAddress (static_stage_resolve, called from swe_mesh_create)
+// and kept in g_static_stage_ptr[device].
+static __device__ __align__(256) double g_static_stage[3 * (size_t)SWE_STATIC_MAX_CELLS];
+constexpr int STATIC_MAX_DEVICES = 64;
+double* g_static_stage_ptr[STATIC_MAX_DEVICES] = {nullptr};
+cudaError_t g_static_stage_err[STATIC_MAX_DEVICES] = {cudaSuccess};
+bool g_static_stage_asked[STATIC_MAX_DEVICES] = {false};
+// set-up, once per device, `dev` current: never allocates; a failure is remembered and reported by
+// the entry point that needs the array (nothing else depends on it)
+void static_stage_resolve(int dev) {
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES || g_static_stage_asked[dev]) return;
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_stage);
+    if (e != cudaSuccess) cudaGetLastError();
+    g_static_stage_ptr[dev] = (e == cudaSuccess) ? (double*)p : nullptr;
+    g_static_stage_err[dev] = e;
+    g_static_stage_asked[dev] = true;
+}
+
 }  // namespace
 
 struct swe_ctx {
     cudaStream_t stream = nullptr;
+    int device = 0;                    // the device that was current in swe_mesh_create
     int num_sm = 148;
     HostMesh H;
     ZoneSet Z;
@@ -532,6 +559,8 @@ int swe_mesh_create(swe_ctx** out, int64_t nv, const double* x, const double* y,
     if (!ok) { delete c; return fail(SWE_ERR_MESH, err); }
     int dev = 0;
     cudaGetDevice(&dev);
+    c->device = dev;
+    static_stage_resolve(dev);         // address of the static staging array on this device (swe_get_state_static)
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) c->num_sm = prop.multiProcessorCount;
     // persistent grids: (resident blocks per SM) x (SM count), from the occupancy calculator
@@ -748,6 +777,46 @@ int swe_get_state(const swe_ctx* cc, double* h, double* hu, double* hv) {
     c->launches++;
     CU(cudaGetLastError());
     if (!dev) {
+        CU(cudaMemcpyAsync(h, dh, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(hu, dhu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(hv, dhv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    return SWE_OK;
+}
+
+int swe_get_state_static(const swe_ctx* cc, double* h, double* hu, double* hv) {
+    KeepMasks keep_masks(cc);   // read-only
+    swe_ctx* c = const_cast<swe_ctx*>(cc);
+    if (check_ctx(c)) return SWE_ERR_ARG;
+    if (!h || !hu || !hv) return fail(SWE_ERR_ARG, "NULL state array");
+    const int64_t nt = c->H.nt;
+    if (nt > (int64_t)SWE_STATIC_MAX_CELLS)
+        return fail(SWE_ERR_ARG, "swe_get_state_static: the mesh has " + std::to_string(nt) + " cells, the static staging array holds at most " +
+                                 std::to_string((long long)SWE_STATIC_MAX_CELLS) + " (SWE_STATIC_MAX_CELLS); use swe_get_state");
+    const int dev = c->device;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES || !g_static_stage_asked[dev] || !g_static_stage_ptr[dev])
+        return fail(SWE_ERR_CUDA, std::string("swe_get_state_static: no device address for the static staging array (cudaGetSymbolAddress: ") +
+                                  ((dev >= 0 && dev < STATIC_MAX_DEVICES && g_static_stage_asked[dev]) ? cudaGetErrorString(g_static_stage_err[dev]) : "not asked for on this device") + ")");
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != dev)
+        return fail(SWE_ERR_STATE, "swe_get_state_static: the context's device must be the current device");
+    const bool devout = is_device_ptr(h) && is_device_ptr(hu) && is_device_ptr(hv);
+    double* stage = g_static_stage_ptr[dev];                // the DEVICE address, not the host-side symbol
+    double *dh = devout ? h : stage, *dhu = devout ? hu : stage + nt, *dhv = devout ? hv : stage + 2 * nt;
+    // Every slot that is copied out below is written first by this call (the array keeps whatever the
+    // last call left there: nothing in it has to start at zero).  Zones distributed over ranks: only
+    // this rank's cells are written, so the caller's other entries are staged in first, as swe_get_state does.
+    if (!devout && c->has_zones && c->Z.nranks > 1) {
+        CU(cudaMemcpyAsync(dh, h, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(dhu, hu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+        CU(cudaMemcpyAsync(dhv, hv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
+    }
+    Store& st = c->active();
+    k_state_to_user<<<grid_for(st.nc, c->grid_light), 256, 0, c->stream>>>(st.A, st.d_cell_user, st.dm.layer, dh, dhu, dhv, (int)st.nc);
+    c->launches++;
+    CU(cudaGetLastError());
+    if (!devout) {
         CU(cudaMemcpyAsync(h, dh, nt * sizeof(double), cudaMemcpyDefault, c->stream));
         CU(cudaMemcpyAsync(hu, dhu, nt * sizeof(double), cudaMemcpyDefault, c->stream));
         CU(cudaMemcpyAsync(hv, dhv, nt * sizeof(double), cudaMemcpyDefault, c->stream));
