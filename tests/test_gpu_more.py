@@ -351,3 +351,57 @@ def test_division_and_square_root_sequences_equal_ieee():
         assert r["div_differs"] == 0 and r["sqrt_differs"] == 0, r
     finally:
         sw.swe_mesh_destroy(c)
+
+
+@pytest.mark.parametrize("ndistinct", [1, 4, 255, 256, 0])
+def test_manning_table_and_per_cell_fallback(ndistinct):
+    """Manning n travels as a one-byte code per cell + a table of the distinct values (at most 255);
+    with more distinct values every cell carries code 255 and the update kernel reads the per-cell
+    array.  Both routes against the oracle (<= 1e-11 per step), un-zoned and with zones created
+    before and after swe_set_manning, device and host pointers.  ndistinct = 0: one value per cell."""
+    import torch
+    cfg = config3(length=1600.0, half_width=400.0, w2=20.0, n4=3, n8=2)
+    nt = cfg["tri"].shape[0]
+    rng = np.random.default_rng(11)
+    if ndistinct == 0:
+        nman = rng.uniform(0.01, 0.06, nt)
+        assert np.unique(nman).size > 255
+    else:
+        vals = np.concatenate([[0.0], rng.uniform(0.01, 0.06, ndistinct - 1)]) if ndistinct > 1 else np.array([0.033])
+        nman = vals[rng.integers(0, ndistinct, nt)]
+        nman[:ndistinct] = vals                                    # every value occurs
+    po.set_threads(0)
+    o = po.Oracle.from_config(cfg)
+    o.set_manning(nman)
+    a = sw.create_from_config(cfg)                                 # un-zoned, host pointer
+    b = sw.create_from_config(cfg)                                 # zones first, then Manning from a device pointer
+    c = sw.create_from_config(cfg)                                 # Manning first, then zones
+    try:
+        sw.swe_set_manning(a, nman)
+        sw.swe_zones_create(b, 4, 2)
+        sw.swe_set_manning(b, torch.tensor(nman, device="cuda"))
+        sw.swe_set_manning(c, nman)
+        sw.swe_zones_create(c, 8, 2)
+        o.step(15, 0.45, "muscl")                                  # water starts to move: friction matters
+        for x in (a, b, c):
+            sw.swe_step(x, 15, 0.45, "muscl")
+        ref = sw.swe_get_state(a)
+        assert_parity(o.get_state(), ref, 1e-9, what="manning %d run" % ndistinct)
+        for x in (b, c):
+            for p, q in zip(ref, sw.swe_get_state(x)):
+                assert np.array_equal(p, q)
+        for s in range(5):
+            sw.swe_set_state(a, *o.get_state())
+            o.step(1, 0.45, "muscl")
+            sw.swe_step(a, 1, 0.45, "muscl")
+            assert_parity(o.get_state(), sw.swe_get_state(a), 1e-11, what="manning %d step %d" % (ndistinct, s))
+        # back to no friction at all, and to a table again: the codes are rewritten every time
+        sw.swe_set_manning(a, None); o.set_manning(None)
+        o.step(3, 0.9, "hllc"); sw.swe_set_state(a, *o.get_state())
+        sw.swe_set_manning(a, np.full(nt, 0.02)); o.set_manning(np.full(nt, 0.02))
+        o.step(1, 0.9, "hllc"); sw.swe_step(a, 1, 0.9, "hllc")
+        assert_parity(o.get_state(), sw.swe_get_state(a), 1e-11, what="manning reset")
+    finally:
+        for x in (a, b, c):
+            sw.swe_mesh_destroy(x)
+        o.close()
