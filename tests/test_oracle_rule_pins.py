@@ -400,3 +400,18 @@ def test_multislope_face_values_on_a_skewed_stencil_worked_from_eq_22_24():
         if checked == 12:
             break
     assert checked == 12 and skew > 0.01                           # the two distances really differ
+
+
+def test_mutation_list_still_applies_to_the_oracle_source():
+    """oracle/mutation_check.py breaks one rule at a time by exact text replacement: every pattern
+    must occur exactly once in oracle/swe_oracle.cpp, or the mutant silently tests nothing (the
+    script reports such a mutant as STALE).  The mutation run itself takes ~10 minutes and is not
+    part of the suite."""
+    import os
+    from oracle import mutation_check as mc
+    src = open(os.path.join(os.path.dirname(mc.__file__), "swe_oracle.cpp")).read()
+    names = [m[0] for m in mc.MUTANTS]
+    assert len(names) == len(set(names)) and len(names) >= 56
+    for name, rule, find, repl in mc.MUTANTS:
+        assert src.count(find) == 1, name
+        assert find != repl and rule
