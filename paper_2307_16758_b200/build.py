@@ -1,7 +1,8 @@
 """Builds the CUDA library in-tree:  python -m paper_2307_16758_b200.build [--force] [--verbose]
 
 nvcc cross-compiles for sm_100a without a GPU.  The host set-up (host_mesh.cpp) is compiled with
--ffp-contract=off so the mesh geometry is the literal IEEE evaluation of its formulas.
+-ffp-contract=off so the mesh geometry is the literal IEEE evaluation of its formulas; OpenMP only
+spreads its independent per-cell / per-edge loops over the host cores (set-up time, not results).
 """
 import os
 import subprocess
@@ -35,12 +36,12 @@ def build(force=False, verbose=False):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
     objs = [os.path.join(CSRC, "%s.%d.o" % (n, os.getpid())) for n in ("host_mesh", "host_inspect")]
-    cmds = [["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-Wall", "-c",
+    cmds = [["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-Wall", "-c",
              os.path.join(CSRC, n + ".cpp"), "-o", o]
             for n, o in zip(("host_mesh", "host_inspect"), objs)]
     cmds.append([NVCC] + ARCH + ["-lineinfo", "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",
                                  "-Xptxas", "-v" if verbose else "-O3"] + EXTRA + [
-                                 os.path.join(CSRC, "swe_api.cu")] + objs + ["-o", tmp, "-lcudart"])
+                                 os.path.join(CSRC, "swe_api.cu")] + objs + ["-o", tmp, "-lcudart", "-lgomp"])
     try:
         for cmd in cmds:
             if verbose:
