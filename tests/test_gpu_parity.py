@@ -256,6 +256,25 @@ def test_config3_full_stated_step_count(scheme, cfl):
         o.close()
 
 
+@pytest.mark.parametrize("scheme,cfl", [("waf", 0.45), ("muscl_ms", 0.45)])
+def test_config3_full_other_schemes_twenty_steps(scheme, cfl):
+    """The two schemes configs[3] does not name (WAF, row a5; the paper's multislope MUSCL, row f1)
+    at full size too, for the 20 steps SURVEY.md 8(d) plans for the oracle at 13.1 M cells: free run
+    from the initial state, per-step bar after step 1, run bar after 20, identical masks."""
+    cfg = config3()
+    o, c = _pair(cfg)
+    try:
+        for chunk, tol in ((1, TOL_STEP), (19, TOL_RUN)):
+            to, _ = o.step(chunk, cfl, scheme)
+            tg, _ = sw.swe_step(c, chunk, cfl, scheme)
+            e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, chunk))
+            print("c3 full %s +%d steps: %s" % (scheme, chunk, e))
+            assert abs(tg - to) <= 1e-11 * to
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
