@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <unordered_map>
 #include <utility>
 #include <map>
 #include <new>
@@ -687,17 +688,21 @@ int swe_set_manning(swe_ctx* c, const double* n_cell) {
         std::vector<double> tab(256, 0.0);
         bool fits = true;
         if (hv) {
-            std::vector<uint64_t> bits;                       // the table, by bit pattern
-            int last = -1;
-            for (int64_t i = 0; i < nt && fits; ++i) {
+            std::unordered_map<uint64_t, int> codes;          // the table, by bit pattern
+            uint64_t last_b = 0; int last = -1;
+            for (int64_t i = 0; i < nt; ++i) {
                 uint64_t b; std::memcpy(&b, &hv[i], 8);
-                int k = (last >= 0 && bits[last] == b) ? last : -1;
-                for (int j = 0; k < 0 && j < (int)bits.size(); ++j) if (bits[j] == b) k = j;
-                if (k < 0) {
-                    if (bits.size() == 255) { fits = false; break; }
-                    k = (int)bits.size(); bits.push_back(b); tab[k] = hv[i];
+                int k;
+                if (last >= 0 && b == last_b) k = last;
+                else {
+                    auto it = codes.find(b);
+                    if (it != codes.end()) k = it->second;
+                    else {
+                        if (codes.size() == 255) { fits = false; break; }
+                        k = (int)codes.size(); codes.emplace(b, k); tab[k] = hv[i];
+                    }
                 }
-                code[i] = (unsigned char)k; last = k;
+                code[i] = (unsigned char)k; last = k; last_b = b;
             }
         }
         if (!fits) std::fill(code.begin(), code.end(), (unsigned char)255);
