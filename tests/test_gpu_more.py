@@ -405,3 +405,39 @@ def test_manning_table_and_per_cell_fallback(ndistinct):
         for x in (a, b, c):
             sw.swe_mesh_destroy(x)
         o.close()
+
+
+def test_dry_counts_and_zone_setup_detail():
+    """swe_dry_counts against numpy on the state the library holds (un-zoned and zoned; bench.py
+    prints these fractions beside the roofline), swe_zone_setup_detail adds up, swe_account_replays
+    moves the counters."""
+    cfg = config3(length=3200.0, half_width=600.0, w2=30.0, n4=4, n8=3)
+    c = sw.create_from_config(cfg)
+    o = po.Oracle.from_config(cfg)
+    try:
+        sw.swe_step(c, 7, 0.45, "muscl")
+        h, hu, hv = sw.swe_get_state(c)
+        eg = o.edge_geometry()
+        inner = eg["eR"] >= 0
+        want_edges = int(np.count_nonzero((h[eg["eL"][inner]] == 0.0) & (h[eg["eR"][inner]] == 0.0)))
+        d = sw.swe_dry_counts(c)
+        assert d["cells"] == h.size and d["interior_edges"] == int(inner.sum())
+        assert d["cells_not_wet"] == int(np.count_nonzero(~(h > 1e-6)))
+        assert d["cells_empty"] == int(np.count_nonzero(h == 0.0)) > 0
+        assert d["edges_between_empty_cells"] == want_edges > 0
+        sw.swe_zones_create(c, 4, 2)
+        dz = sw.swe_dry_counts(c)                                    # owned cells of the zoned copy
+        assert dz["cells_not_wet"] == d["cells_not_wet"] and dz["cells_empty"] == d["cells_empty"]
+        t = sw.swe_zone_setup_detail(c)
+        parts = t["zone_of_ms"] + t["ghost_layers_ms"] + t["lists_ms"] + t["assembly_ms"]
+        assert all(v >= 0.0 for v in t.values()) and parts <= t["total_ms"] * 1.001 and t["assembly_ms"] > 0.0
+        s0 = sw.swe_get_stats(c)
+        sw.swe_account_replays(c, 3, 39, 1000)
+        s1 = sw.swe_get_stats(c)
+        assert (s1["steps"] - s0["steps"], s1["kernel_launches"] - s0["kernel_launches"],
+                s1["halo_bytes"] - s0["halo_bytes"]) == (3, 39, 1000)
+        sw.swe_account_replays(c, -3, -39, -1000)
+        assert sw.swe_get_stats(c) == s0
+    finally:
+        sw.swe_mesh_destroy(c)
+        o.close()

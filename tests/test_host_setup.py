@@ -265,3 +265,14 @@ def test_third_offset_travels_as_a_single_precision_residual():
                 assert (back == r2).mean() > 0.999
             finally:
                 sw.swe_host_mesh_free(h)
+
+
+def test_build_check_fails_loudly_when_a_source_is_missing(monkeypatch):
+    """A library next to an incomplete source tree must not be picked up silently
+    (paper_2307_16758_b200/build.py needs_build)."""
+    from paper_2307_16758_b200 import build as b
+    assert b.needs_build() is False                       # the suite runs on a freshly built library
+    monkeypatch.setattr(b, "DEPS", list(b.DEPS) + ["no_such_file.cuh"])
+    with pytest.raises(FileNotFoundError) as e:
+        b.needs_build()
+    assert "no_such_file.cuh" in str(e.value)
