@@ -415,3 +415,56 @@ def test_mutation_list_still_applies_to_the_oracle_source():
     for name, rule, find, repl in mc.MUTANTS:
         assert src.count(find) == 1, name
         assert find != repl and rule
+
+
+# ---------------------------------------------------------------------------------------------
+# A.10: h' = max(h', 0), whatever the time step
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("scheme", ["hllc", "muscl", "waf", "muscl_ms"])
+def test_a_stage_never_returns_a_negative_depth_whatever_the_time_step(scheme):
+    """A.10 clamps the updated depth at zero and zeroes the momentum of a cell that ends up not wet.
+    At the CFL numbers the schemes are run with, the hydrostatic reconstruction keeps depths positive
+    by itself and the clamp never acts; a stage with forty times the stable time step drains cells
+    below zero, and the rule must still hold: no negative depth, no momentum without water."""
+    cfg = si.config0(nx=60, ny=4, h_left=2.0, h_right=0.02)
+    o = po.Oracle.from_config(cfg)
+    o.step(5, 0.45, "hllc")                                        # a moving front
+    dt = 40.0 * o.compute_dt(0.9)
+    h, hu, hv = o.euler_stage(dt, scheme)
+    assert np.all(np.isfinite(h)) and np.all(np.isfinite(hu)) and np.all(np.isfinite(hv))
+    assert h.min() >= 0.0
+    assert (h == 0.0).any()                                        # the clamp was needed somewhere
+    dry = h <= 1e-6
+    assert np.all(hu[dry] == 0.0) and np.all(hv[dry] == 0.0)
+
+
+# ---------------------------------------------------------------------------------------------
+# R11: the level boundary's ghost depth stands over the FACE bed
+# ---------------------------------------------------------------------------------------------
+def test_lake_at_rest_against_a_level_boundary_with_unlimited_gradients():
+    """C-property at the open boundary.  With z_ghost = z_f (A.8) a lake at rest at the imposed
+    level sees its own face state in the ghost -- h_b = level - z_f = h_f -- and nothing moves,
+    however the depth is reconstructed.  The cell limiter hides this at boundary cells (they are
+    local extrema among their two real neighbours, so their limited gradient is zero and
+    z_f = z_cell); with unlimited gradients (beta <= 0) over an uneven bed the face bed differs from
+    the cell bed by centimetres, and a ghost standing over the CELL bed would drive a flow."""
+    x, y, tri = si.grid_mesh(20, 4, 20.0, 4.0, 0.15, 11)
+    be = si.boundary_edges(tri)
+    xm = 0.5 * (x[be[:, 0]] + x[be[:, 1]])
+    east = be[xm > 20.0 - 1e-9]
+    zb = 0.2 * np.sin(x) + 0.1 * y + 0.03 * x
+    o = po.Oracle(x, y, zb, tri, east, np.full(len(east), 2, np.int32))
+    o.set_bc(2, "level", 3.0)
+    o.set_params(beta=0.0)
+    zc = o.cell_geometry()["zc"]
+    h0 = 3.0 - zc
+    o.set_state(h0, np.zeros(o.nt), np.zeros(o.nt))
+    gr = o.gradients()
+    c2c, _ = o.cell_topology()
+    cx = x[tri].mean(axis=1)
+    at_outlet = (cx > 19.0) & ((c2c < 0).sum(axis=1) >= 1)
+    assert np.abs(gr[at_outlet, 2:4]).max() > 0.02                 # the depth gradient is alive there
+    o.step(40, 0.45, "muscl")
+    h, hu, hv = o.get_state()
+    assert np.abs(hu / h).max() <= 1e-12 and np.abs(hv / h).max() <= 1e-12
+    assert np.abs(h - h0).max() <= 1e-12
