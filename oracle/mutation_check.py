@@ -10,7 +10,8 @@ failure.  A mutant that passes every pin is reported as SURVIVED: the rule it br
 and belongs in the "parity unpinned" list of DESIGN.md section 2.  Nothing in the repository is
 modified; nothing under paper_2307_16758_b200/ is touched or loaded.
 
-The list starts with the seven mutants of VERDICT.md (round 1) "What's weak" 1.
+The list starts with the seven mutants of VERDICT.md (round 1) "What's weak" 1; 74 in all.  One is
+expected to survive and is declared unpinned in DESIGN.md section 2 (`manning_uses_old_depth`).
 """
 import argparse
 import os
@@ -21,7 +22,8 @@ import tempfile
 import time
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-TIMEOUT_S = 600          # per mutant
+TIMEOUT_S = 900          # per mutant
+TEST_TIMEOUT_S = 240     # per test (the slowest pin takes 25 s on 8 cores when the oracle is intact)
 
 # (name, rule broken, exact text to find, replacement)
 MUTANTS = [
@@ -169,7 +171,8 @@ def run_one(name, find, repl, tests, keep):
         # (the guard test that checks this list against the UNMUTATED source would "kill" every mutant)
         try:
             r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-m", "not gpu", "-p", "no:cacheprovider",
-                            "-k", "not test_mutation_list_still_applies_to_the_oracle_source"]
+                            "-k", "not test_mutation_list_still_applies_to_the_oracle_source",
+                            "--timeout", str(TEST_TIMEOUT_S)]     # pytest-timeout: a pin that does not come back fails by name
                            + [os.path.join("tests", t) for t in tests],
                                cwd=tmp, env=env, capture_output=True, text=True, timeout=TIMEOUT_S)
         except subprocess.TimeoutExpired:

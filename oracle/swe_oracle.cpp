@@ -27,13 +27,18 @@
 // the order k=0,1,2 and updates).  Both cells of an edge evaluate bit-identical fluxes, so mass is
 // conserved to round-off without a flux buffer.  No blocking, fusion or reordering.
 //
-// The open boundaries (inflow Q: sign, magnitude, distribution over the tag's width; fixed level:
-// ghost depth and outgoing Riemann invariant) are pinned by tests/test_oracle_boundaries.py
-// (uniform flow preserved to round-off, relaxation to the backwater curve of the
-// gradually-varied-flow ODE, reflection of a small long wave with coefficient -1).
+// Every rule of this file is pinned by tests/test_oracle_*.py against something the paper or the
+// mathematics fixes (closed forms, invariants, exactness properties, the paper's printed tables;
+// DESIGN.md section 2 lists what pins what), and the pins are checked by mutation
+// (oracle/mutation_check.py: 74 single-rule mutants of this file, 73 killed).
 // PARITY UNPINNED (only oracle<->GPU agreement and mass balance check these):
-//   the momentum part of the inflow flux on dry faces, the WAF Delta-x choice on triangles, the
-//   values of h_dry / h_thin, the WAF->HLLC fallback rule.
+//   * edge_flux, inflow boundary: the momentum part of the flux on DRY faces (q^2/h dropped when
+//     h* <= h_dry, reading R10); its mass part is pinned;
+//   * ratio_r: r = 1 when |Delta_loc| is at round-off (reading R9; the three fluxes coincide there);
+//   * cell_update: WHICH depth enters the Manning factor (the updated h', A.10); the depth before the
+//     update is an equally consistent splitting and coincides with it at every steady state;
+//   * the VALUES of h_dry and h_thin (parameters; that the two thresholds are distinct and which
+//     rule uses which is pinned).
 #include <algorithm>
 #include <cmath>
 #include <cstdint>

@@ -468,3 +468,56 @@ def test_lake_at_rest_against_a_level_boundary_with_unlimited_gradients():
     h, hu, hv = o.get_state()
     assert np.abs(hu / h).max() <= 1e-12 and np.abs(hv / h).max() <= 1e-12
     assert np.abs(h - h0).max() <= 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# eq. 15-17: the Courant numbers c_k = S_k dt / dx inside the edge flux
+# ---------------------------------------------------------------------------------------------
+def test_waf_edge_flux_with_unit_ratios_is_eq17_with_c_from_dt_over_dx():
+    """Upwind cells set so that every limiter ratio is exactly 1 (q_L - q_Lupw = q_R - q_L =
+    q_Rupw - q_R for eta and for the velocity vector): SUPERBEE then gives A = |c| (eq. 21, middle
+    branch) and the WAF flux is the paper's eq. 16-17 with weights (1 +- c_k)/2,
+        G = G* + (1 + c_L)/2 (G_L - G*) + (1 - c_R)/2 (G_R - G*),   G_3 = G_1 [(1 + c_*)/2 v_L + (1 - c_*)/2 v_R],
+    c_k = S_k dt / dx.  The wave speeds and G* come from the HLLC routine (pinned on its own), dx and
+    the normal from the edge geometry (pinned on its own): what is checked is that the edge flux puts
+    them together with THIS dt and THIS dx -- half the time step or another length fails."""
+    x, y, tri = si.grid_mesh(10, 8, 10.0, 8.0, 0.2, 41)
+    o = po.Oracle(x, y, np.zeros_like(x), tri)
+    c2c, _ = o.cell_topology()
+    e = o.edge_geometry()
+    rng = np.random.default_rng(9)
+    inner = np.nonzero(e["eR"] >= 0)[0]
+    checked = 0
+    for ed in rng.permutation(inner):
+        L, R = int(e["eL"][ed]), int(e["eR"][ed])
+        upL = [int(n) for n in c2c[L] if n != R]
+        upR = [int(n) for n in c2c[R] if n != L]
+        if min(upL + upR) < 0 or len(set(upL + upR)) != 4:
+            continue
+        n1, n2, length, dx = e["nx"][ed], e["ny"][ed], e["len"][ed], e["dx"][ed]
+        h = np.full(o.nt, 2.0); u = np.zeros(o.nt); v = np.zeros(o.nt)
+        qL = np.array([2.0, 0.30, -0.10]); qR = np.array([1.7, 0.45, 0.05])        # (h, u, v), subcritical
+        for cells, q in ((([L]), qL), ([R], qR), (upL, qL - (qR - qL)), (upR, qR + (qR - qL))):
+            h[cells], u[cells], v[cells] = q
+        o.set_state(h, h * u, h * v)
+        unL, utL = qL[1] * n1 + qL[2] * n2, -qL[1] * n2 + qL[2] * n1                # eq. 2
+        unR, utR = qR[1] * n1 + qR[2] * n2, -qR[1] * n2 + qR[2] * n1
+        w = po.hllc(G, 1e-6, qL[0], unL, utL, qR[0], unR, utR)
+        assert w["SL"] < 0.0 < w["SR"] and abs(w["Sstar"]) > 1e-3                   # G = G* for HLLC here
+        dt = 0.4 * dx / max(abs(w["SL"]), abs(w["SR"]))
+        cL, cR, cS = w["SL"] * dt / dx, w["SR"] * dt / dx, w["Sstar"] * dt / dx
+        GL = np.array([qL[0] * unL, qL[0] * unL ** 2 + 0.5 * G * qL[0] ** 2])       # eq. 1, normal frame
+        GR = np.array([qR[0] * unR, qR[0] * unR ** 2 + 0.5 * G * qR[0] ** 2])
+        Gs = np.array([w["G1"], w["G2"]])
+        Gw = Gs + 0.5 * (1.0 + cL) * (GL - Gs) + 0.5 * (1.0 - cR) * (GR - Gs)
+        G3 = Gw[0] * (0.5 * (1.0 + cS) * utL + 0.5 * (1.0 - cS) * utR)
+        bL = Gw[1] - 0.5 * G * qL[0] ** 2                                           # A.9, first-order faces, flat bed
+        want = length * np.array([Gw[0], bL * n1 - G3 * n2, bL * n2 + G3 * n1])
+        got = o.edge_flux(ed, dt, "waf")[0]
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-12 * np.abs(want).max())
+        half = o.edge_flux(ed, 0.5 * dt, "waf")[0]
+        assert np.abs(half - want).max() > 1e-3 * np.abs(want).max()
+        checked += 1
+        if checked == 10:
+            break
+    assert checked == 10
