@@ -163,10 +163,15 @@ class DistSolver:
     nlayers ghost layers (>= 2 for MUSCL / WAF / MUSCL_MS); transport "p2p" (peer-memory push, one
     kernel per exchange) or "staged" (pack -> all-to-all -> unpack).
 
-    Streams: the context runs on the torch stream that is current when the solver is created, and
-    the stream-ordered collectives that order the halo pushes against the peers' ghost reads are
-    enqueued on torch's current stream: the two must be the same stream, so step() and exchange()
-    raise if they are called under another one.
+    Streams: the solver owns a CUDA stream; the library context is created on it and every library
+    call and every collective is issued under it, because the stream-ordered collectives that order
+    the halo pushes against the peers' ghost reads only do so on ONE stream.  step(), exchange(),
+    set_state() and the getters order that stream behind the caller's current torch stream on entry
+    and the caller's stream behind it on exit, so a caller may use any stream.
+
+    graphs=True (nccl backend): one step is captured once per (scheme, cfl) as a CUDA graph --
+    kernels and collectives alike -- and replayed; the ranks agree on whether the capture worked and
+    fall back to call-by-call steps together if it did not on any of them.
     """
 
     def __init__(self, cfg, nzones=None, nlayers=2, transport="p2p", zone_of_cell=None, comm=None,
@@ -398,6 +403,19 @@ class DistSolver:
                     body(sch, cfl)                         # a real step: NCCL set-up and lazy loading happen outside the capture
                     done = 1
                     ent = self._capture(body, sch, cfl)
+                    # every rank or none: a rank whose capture failed has neither run nor recorded the
+                    # step, the others have only recorded it, so nobody has executed anything yet and
+                    # all can still fall back to enqueuing call by call together (one-time host sync)
+                    ok = self.torch.tensor([1.0 if ent is not None else 0.0], dtype=self.torch.float64,
+                                           device=self.minbuf.device)
+                    self.comm.allreduce_min(ok)
+                    if float(ok.item()) < 1.0:
+                        if ent is not None:
+                            import sys
+                            sys.stderr.write("[swe dist] rank %d: another rank could not capture the step as a CUDA "
+                                             "graph; steps are enqueued call by call\n" % self.rank)
+                        ent = None
+                        self.graphs = False
                     if ent is not None:
                         self._graph[key] = ent
                 if ent is not None:
@@ -422,6 +440,9 @@ class DistSolver:
         s1 = sw.swe_get_stats(self.ctx)
         try:
             with torch.cuda.graph(g, stream=self.tstream, capture_error_mode="thread_local"):
+                if os.environ.get("SWE_DIST_GRAPH_FAIL"):      # test hook: a capture that breaks half way
+                    self.sw.swe_dist_begin_step(self.ctx, self.minbuf, cfl)
+                    raise RuntimeError("SWE_DIST_GRAPH_FAIL is set")
                 body(sch, cfl)
         except Exception as e:                             # depends on the NCCL build
             import sys

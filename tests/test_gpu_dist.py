@@ -312,6 +312,17 @@ def _nccl_worker(port, schedule, transport, q):
         S2.close()
         assert S2.graph_replays == 0 and t_eager == t and all(np.array_equal(x, y) for x, y in zip(st, st_eager))
         assert stats2["kernel_launches"] == stats["kernel_launches"] and stats2["halo_bytes"] == stats["halo_bytes"], (stats, stats2)
+        # a capture that fails half way: every rank falls back to call-by-call steps, nothing is lost
+        os.environ["SWE_DIST_GRAPH_FAIL"] = "1"
+        S3 = d.DistSolver(cfg, nzones=4, nlayers=2, transport=transport, schedule=schedule)
+        S3.step(8, 0.45, "muscl"); S3.step(7, 0.9, "hllc"); S3.step(5, 0.45, "waf")
+        del os.environ["SWE_DIST_GRAPH_FAIL"]
+        st_fb, t_fb = S3.get_state(), S3.time()
+        stats3 = sw.swe_get_stats(S3.ctx)
+        S3.close()
+        assert S3.graph_replays == 0 and S3.graphs is False and t_fb == t
+        assert all(np.array_equal(x, y) for x, y in zip(st, st_fb)), "fallback after a failed capture"
+        assert stats3["steps"] == 20 and stats3["kernel_launches"] == stats["kernel_launches"], (stats, stats3)
         S.set_state(*[torch.from_numpy(x.copy()) for x in st])
         S.step(3, 0.45, "muscl_ms")
         st2 = S.get_state()
