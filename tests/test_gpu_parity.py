@@ -195,8 +195,9 @@ def test_config2_full(scheme):
             o.step(chunk, 0.45, scheme)
             sw.swe_step(c, chunk, 0.45, scheme)
             done += chunk
-            assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP if done == 1 else TOL_RUN,
-                          what="c2 %s after %d steps" % (scheme, done))
+            e = assert_parity(o.get_state(), sw.swe_get_state(c), TOL_STEP if done == 1 else TOL_RUN,
+                              what="c2 %s after %d steps" % (scheme, done))
+            print("c2 full %s after %d steps: %s" % (scheme, done, e))
         assert abs(sw.swe_get_time(c)[0] - o.step(0, 0.45, scheme)[0]) <= 1e-12 * sw.swe_get_time(c)[0]
         for h, hu, hv in (sw.swe_get_state(c), o.get_state()):
             wet = h > 1e-6
