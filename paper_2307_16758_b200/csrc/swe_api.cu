@@ -14,6 +14,7 @@
 #include <unordered_map>
 #include <utility>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -97,7 +98,9 @@ cudaError_t g_static_stage_err[STATIC_MAX_DEVICES] = {cudaSuccess};
 bool g_static_stage_asked[STATIC_MAX_DEVICES] = {false};
 // set-up, once per device, `dev` current: never allocates; a failure is remembered and reported by
 // the entry point that needs the array (nothing else depends on it)
+std::mutex g_static_stage_mutex;           // two threads may create their first contexts at the same time
 void static_stage_resolve(int dev) {
+    std::lock_guard<std::mutex> lock(g_static_stage_mutex);
     if (dev < 0 || dev >= STATIC_MAX_DEVICES || g_static_stage_asked[dev]) return;
     void* p = nullptr;
     const cudaError_t e = cudaGetSymbolAddress(&p, g_static_stage);
