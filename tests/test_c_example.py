@@ -37,3 +37,4 @@ def test_c_example_runs_on_the_gpu(tmp_path):
     out = subprocess.run([exe], capture_output=True, text=True, timeout=300)
     assert out.returncode == 0, out.stdout + out.stderr
     assert "HLLC" in out.stdout and "MUSCL-RK2" in out.stdout and "mass drift" in out.stdout
+    assert "8 zones x 2 layers" in out.stdout and "bit-identical to the un-zoned run" in out.stdout
