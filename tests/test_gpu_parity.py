@@ -229,8 +229,26 @@ def test_config3_reduced_long_run():
             o.close()
 
 
+@pytest.fixture(scope="module")
+def c3_full():
+    """configs[3] at full size, built ONCE for the full-size tests below (generator 7 s, the
+    oracle's mesh 8 s, swe_mesh_create 6.5 s): every test restarts both sides from the initial state."""
+    cfg = config3()
+    o, c = _pair(cfg)
+    assert o.nt > 12_000_000
+    yield cfg, o, c
+    sw.swe_mesh_destroy(c)
+    o.close()
+
+
+def _restart(cfg, o, c):
+    o.set_state(cfg["h"], cfg["hu"], cfg["hv"])
+    sw.swe_set_state(c, cfg["h"], cfg["hu"], cfg["hv"])
+    return o.step(0, 0.9, "hllc")[0], sw.swe_get_time(c)[0]          # the two clocks at the restart
+
+
 @pytest.mark.parametrize("scheme,cfl", [("muscl", 0.45), ("hllc", 0.9)])
-def test_config3_full_stated_step_count(scheme, cfl):
+def test_config3_full_stated_step_count(c3_full, scheme, cfl):
     """configs[3] at full size (13.1 M cells), in the launch configuration bench.py times, for the
     stated 200 steps with the oracle running all of them beside the GPU (20 steps,
     "all 200 if the OpenMP oracle needs < 10 min": it needs 40 s for HLLC, 130 s for MUSCL on the
@@ -239,41 +257,32 @@ def test_config3_full_stated_step_count(scheme, cfl):
     Measured (round 2): MUSCL 2e-15 after 200 steps; HLLC 2e-14 until step 190 and 4e-10 at step
     200, where one wet/dry front decision falls on different steps on the two sides (DESIGN.md
     section 3) -- inside the 1e-8 bar."""
-    cfg = config3()
-    o, c = _pair(cfg)
-    try:
-        assert o.nt > 12_000_000
-        done = 0
-        for chunk in (1, 1, 18, 80, 100):
-            to, _ = o.step(chunk, cfl, scheme)
-            tg, _ = sw.swe_step(c, chunk, cfl, scheme)
-            done += chunk
-            tol = TOL_STEP if done == 1 else TOL_RUN
-            e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, done))
-            print("c3 full %s after %d steps: %s" % (scheme, done, e))
-            assert abs(tg - to) <= 1e-11 * to
-    finally:
-        sw.swe_mesh_destroy(c)
-        o.close()
+    cfg, o, c = c3_full
+    to0, tg0 = _restart(cfg, o, c)
+    done = 0
+    for chunk in (1, 1, 18, 80, 100):
+        to, _ = o.step(chunk, cfl, scheme)
+        tg, _ = sw.swe_step(c, chunk, cfl, scheme)
+        done += chunk
+        tol = TOL_STEP if done == 1 else TOL_RUN
+        e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, done))
+        print("c3 full %s after %d steps: %s" % (scheme, done, e))
+        assert abs((tg - tg0) - (to - to0)) <= 1e-11 * (to - to0)
 
 
 @pytest.mark.parametrize("scheme,cfl", [("waf", 0.45), ("muscl_ms", 0.45)])
-def test_config3_full_other_schemes_twenty_steps(scheme, cfl):
+def test_config3_full_other_schemes_twenty_steps(c3_full, scheme, cfl):
     """The two schemes configs[3] does not name (WAF, row a5; the paper's multislope MUSCL, row f1)
     at full size too, for the 20 steps SURVEY.md 8(d) plans for the oracle at 13.1 M cells: free run
     from the initial state, per-step bar after step 1, run bar after 20, identical masks."""
-    cfg = config3()
-    o, c = _pair(cfg)
-    try:
-        for chunk, tol in ((1, TOL_STEP), (19, TOL_RUN)):
-            to, _ = o.step(chunk, cfl, scheme)
-            tg, _ = sw.swe_step(c, chunk, cfl, scheme)
-            e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, chunk))
-            print("c3 full %s +%d steps: %s" % (scheme, chunk, e))
-            assert abs(tg - to) <= 1e-11 * to
-    finally:
-        sw.swe_mesh_destroy(c)
-        o.close()
+    cfg, o, c = c3_full
+    to0, tg0 = _restart(cfg, o, c)
+    for chunk, tol in ((1, TOL_STEP), (19, TOL_RUN)):
+        to, _ = o.step(chunk, cfl, scheme)
+        tg, _ = sw.swe_step(c, chunk, cfl, scheme)
+        e = assert_parity(o.get_state(), sw.swe_get_state(c), tol, what="c3 %s after %d steps" % (scheme, chunk))
+        print("c3 full %s +%d steps: %s" % (scheme, chunk, e))
+        assert abs((tg - tg0) - (to - to0)) <= 1e-11 * (to - to0)
 
 
 # ---------------------------------------------------------------------------------------------
